@@ -1,0 +1,137 @@
+/*
+ * lqcd.h -- C ABI of the B200-native Wilson dslash library (liblqcd.so).
+ *
+ * The hot path of "LatticeQCD using OpenCL" (arXiv:1112.5280): the Wilson hopping
+ * operator ("the non-diagonal part of the Dirac matrix ('dslash')", sec. 3),
+ * in full and even-odd preconditioned form (Fig. 5 caption), and the
+ * fermion matrix M built on it ("M is the fermion matrix", sec. 4).
+ * The paper prints no formula; the definition is the textbook Wilson form fixed in
+ * SURVEY.md sec. 8(c) / Appendix A and restated in DESIGN.md:
+ *
+ *   (H psi)(x) = sum_{mu=0..3} [ (1 - gamma_mu) U_mu(x)         psi(x + mu^)
+ *                              + (1 + gamma_mu) U_mu(x - mu^)^+  psi(x - mu^) ]
+ *   M_full = 1 - kappa H ;   M_eo = 1 - kappa^2 H_eo H_oe  on even sites
+ *   psi(x + L_mu mu^) = bc_mu psi(x),  |bc_mu| = 1   (phase applied at the crossing hop only)
+ *
+ * mu = 0,1,2,3 = x,y,z,t; parity p(x) = (x+y+z+t) & 1; chiral gamma basis of DESIGN.md.
+ *
+ * General rules for every entry point
+ *   - Pointers named *_dev are CUDA device pointers, *_host are host pointers.  The caller
+ *     (PyTorch) allocates and frees every buffer; the library allocates no field memory and
+ *     keeps no pointer after a call returns.  lqcd_ctx is host memory owned by the library.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
+ *     entry points only enqueue work and return; they never synchronise.  The *_host entry
+ *     point synchronises `stream` before returning (its results live in host memory).
+ *   - All device field pointers must be 16-byte aligned (LQCD_EALIGN otherwise).
+ *   - The stencil is not in-place safe: `out` overlapping `in` / `workspace` gives LQCD_EALIAS.
+ *   - Errors are return codes only: nothing throws, aborts or prints.
+ *
+ * Layouts (element type = float for precision 32, double for precision 64)
+ *   canonical (interchange; complex interleaved re,im; C-contiguous; what torch.complex64/128 holds)
+ *     full spinor  [T][Z][Y][X][spin 4][colour 3]
+ *     half spinor  [V/2][spin 4][colour 3]  -- the sites of one parity in increasing
+ *                  lexicographic order lex = x + X(y + Y(z + Z t)), i.e. indexed by cb = lex >> 1
+ *     links        [mu 4][T][Z][Y][X][row 3][col 3],  (U psi)_a = sum_b U[a][b] psi_b,  U_mu(x) at x
+ *   native (what the hot path reads/writes; structure of arrays, site-fastest, checkerboarded)
+ *     real component r = 6 spin + 2 colour + reim (spinor, 24) or 6 row + 2 col + reim (link,
+ *     first `recon` reals of 18).  W = 16 bytes / sizeof(element) reals per 128-bit word.
+ *     half spinor  word q = r / W, lane = r % W  at  element index (q * V/2 + cb) * W + lane
+ *     full spinor  [even half | odd half]
+ *     links        [parity of base site 2][mu 4][word][V/2][lane]; words of 4 floats (recon 12,
+ *                  3 words), 2 floats (precision 32 recon 18, 9 words of 8 bytes) or 2 doubles.
+ */
+#ifndef LQCD_H
+#define LQCD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lqcd_ctx lqcd_ctx; /* opaque: geometry + constants, host memory */
+
+typedef enum {
+    LQCD_OK = 0,
+    LQCD_EINVAL = 1,       /* null pointer, bad extent / parity / precision / recon, |bc| != 1 */
+    LQCD_EALIGN = 2,       /* a device pointer is not 16-byte aligned */
+    LQCD_EALIAS = 3,       /* out overlaps in or workspace */
+    LQCD_EUNSUPPORTED = 4, /* combination not compiled in */
+    LQCD_ECUDA = 5         /* CUDA runtime / launch error */
+} lqcd_status;
+
+typedef struct {
+    int dims[4];      /* X,Y,Z,T (mu = 0..3); each even and >= 4 (reading A17) */
+    int precision;    /* 32 or 64: storage and arithmetic type of all fields */
+    int recon;        /* 18 or 12: stored reals per link; 12 = two rows, third rebuilt in
+                         registers as conj(row0 x row1) ("RECONSTRUCT TWELVE") */
+    double bc_re[4];  /* boundary phase bc_mu = bc_re + i bc_im, |bc_mu| = 1 within 1e-12; */
+    double bc_im[4];  /* periodic (1,0), antiperiodic (-1,0), any U(1) phase allowed        */
+} lqcd_params;
+
+#define LQCD_PARITY_EVEN 0
+#define LQCD_PARITY_ODD 1
+#define LQCD_PARITY_BOTH (-1)
+
+/* Validate p, copy it; *ctx is set on LQCD_OK only. */
+lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p);
+lqcd_status lqcd_destroy(lqcd_ctx* ctx); /* NULL is a no-op */
+
+/* Sizes in bytes of native buffers for this ctx (0 if ctx is NULL). */
+size_t lqcd_spinor_bytes(const lqcd_ctx* ctx, int half); /* half != 0: one parity; 0: full [even|odd] */
+size_t lqcd_gauge_bytes(const lqcd_ctx* ctx);            /* native links, 2*4*recon*V/2 elements */
+size_t lqcd_workspace_bytes(const lqcd_ctx* ctx);        /* lqcd_apply_M(eo=1): one native half spinor */
+size_t lqcd_host_workspace_bytes(const lqcd_ctx* ctx);   /* device scratch of lqcd_dslash_eo_host */
+
+/* canonical <-> native conversion kernels (layout only, no arithmetic; not on the timed path).
+ * All pointers are device pointers; asynchronous on `stream`.
+ * parity = LQCD_PARITY_EVEN/ODD: canonical half spinor <-> native half spinor;
+ * parity = LQCD_PARITY_BOTH:     canonical full spinor <-> native full spinor [even|odd]. */
+lqcd_status lqcd_pack_gauge(const lqcd_ctx* ctx, void* native_dev, const void* canonical_dev, void* stream);
+lqcd_status lqcd_pack_spinor(const lqcd_ctx* ctx, void* native_dev, const void* canonical_dev, int parity,
+                             void* stream);
+lqcd_status lqcd_unpack_spinor(const lqcd_ctx* ctx, void* canonical_dev, const void* native_dev, int parity,
+                               void* stream);
+
+/* ---- hot path: device pointers, native layout ---- */
+
+/* out = H in on all sites; in/out native full spinors.  One launch. */
+lqcd_status lqcd_dslash_full(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
+                             void* stream);
+
+/* out_p = H_{p,1-p} in_{1-p}: in is a native half spinor of parity 1-out_parity, out one of parity
+ * out_parity (0: H_eo, odd in -> even out; 1: H_oe).  One launch.  No kappa (pure H, so the
+ * 1320 flop/site convention is exact; reading A7). */
+lqcd_status lqcd_dslash_eo(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
+                           int out_parity, void* stream);
+
+/* eo = 0: out = in - kappa H in, native full spinors, one launch, workspace unused (may be NULL).
+ * eo = 1: out_e = in_e - kappa^2 H_eo H_oe in_e, native even half spinors; two launches;
+ *         workspace_dev holds the intermediate odd half spinor (lqcd_workspace_bytes). */
+lqcd_status lqcd_apply_M(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
+                         double kappa, int eo, void* workspace_dev, void* stream);
+
+/* End-to-end convenience for host-resident data: canonical host buffers in, canonical host
+ * buffer out.  Copies gauge_host (canonical links; may be NULL to reuse the links packed into
+ * workspace_dev by an earlier call) and in_host (canonical half spinor of parity 1-out_parity)
+ * to the device, packs, runs lqcd_dslash_eo, unpacks, copies the canonical half spinor of
+ * parity out_parity to out_host and synchronises `stream`.  workspace_dev is device scratch
+ * of lqcd_host_workspace_bytes bytes, 256-byte aligned, owned by the caller.  Host buffers
+ * should be pinned for full PCIe speed (pageable memory works, slower). */
+lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* ctx, void* out_host, const void* gauge_host,
+                                const void* in_host, int out_parity, void* workspace_dev, void* stream);
+
+/* Number of kernels this library has launched since load (a claim counter for bench.py). */
+unsigned long long lqcd_launch_count(void);
+
+/* Launch-geometry knobs for tuning runs; 0 restores the default.  Returns LQCD_EINVAL if the
+ * value is not supported.  block_threads in {64,128,256}. */
+lqcd_status lqcd_set_block_threads(lqcd_ctx* ctx, int block_threads);
+
+const char* lqcd_status_string(lqcd_status s);
+const char* lqcd_last_cuda_error(void); /* text of the last CUDA error seen by this thread's calls */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQCD_H */

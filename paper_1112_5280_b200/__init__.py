@@ -1,0 +1,169 @@
+"""paper_1112_5280_b200 -- B200-native Wilson dslash (arXiv:1112.5280 hot path).
+
+Thin ctypes binding of the C ABI in include/lqcd.h (same names, argument marshalling only:
+every step of the path runs in the CUDA kernels of csrc/).  PyTorch supplies device memory
+and streams.  There is no CPU fallback: if liblqcd.so cannot be loaded the import of any
+entry point raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import _build
+
+LQCD_OK, LQCD_EINVAL, LQCD_EALIGN, LQCD_EALIAS, LQCD_EUNSUPPORTED, LQCD_ECUDA = range(6)
+PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, -1
+
+EXPORTS = [
+    "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
+    "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
+    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_dslash_eo_host", "lqcd_launch_count",
+    "lqcd_set_block_threads", "lqcd_status_string", "lqcd_last_cuda_error",
+]
+
+
+class lqcd_params(ctypes.Structure):
+    _fields_ = [("dims", ctypes.c_int * 4), ("precision", ctypes.c_int), ("recon", ctypes.c_int),
+                ("bc_re", ctypes.c_double * 4), ("bc_im", ctypes.c_double * 4)]
+
+
+class LqcdError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = _lib().lqcd_status_string(status).decode()
+        if status == LQCD_ECUDA:
+            msg += ": " + _lib().lqcd_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} (status {status})")
+
+
+_LIB = None
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        path = _build.LIB
+        if not os.path.exists(path):
+            raise RuntimeError(f"{path} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                               "(the CUDA library is the only implementation; there is no fallback)")
+        lib = ctypes.CDLL(path)
+        vp, ci, cd, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+        lib.lqcd_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(lqcd_params)]
+        lib.lqcd_destroy.argtypes = [vp]
+        for n in ("lqcd_gauge_bytes", "lqcd_workspace_bytes", "lqcd_host_workspace_bytes"):
+            getattr(lib, n).argtypes = [vp]
+            getattr(lib, n).restype = sz
+        lib.lqcd_spinor_bytes.argtypes = [vp, ci]
+        lib.lqcd_spinor_bytes.restype = sz
+        lib.lqcd_pack_gauge.argtypes = [vp, vp, vp, vp]
+        lib.lqcd_pack_spinor.argtypes = [vp, vp, vp, ci, vp]
+        lib.lqcd_unpack_spinor.argtypes = [vp, vp, vp, ci, vp]
+        lib.lqcd_dslash_full.argtypes = [vp, vp, vp, vp, vp]
+        lib.lqcd_dslash_eo.argtypes = [vp, vp, vp, vp, ci, vp]
+        lib.lqcd_apply_M.argtypes = [vp, vp, vp, vp, cd, ci, vp, vp]
+        lib.lqcd_dslash_eo_host.argtypes = [vp, vp, vp, vp, ci, vp, vp]
+        lib.lqcd_launch_count.argtypes = []
+        lib.lqcd_launch_count.restype = ctypes.c_ulonglong
+        lib.lqcd_set_block_threads.argtypes = [vp, ci]
+        lib.lqcd_status_string.argtypes = [ci]
+        lib.lqcd_status_string.restype = ctypes.c_char_p
+        lib.lqcd_last_cuda_error.argtypes = []
+        lib.lqcd_last_cuda_error.restype = ctypes.c_char_p
+        _LIB = lib
+    return _LIB
+
+
+def _ptr(t):
+    """Device/host address of a torch tensor, a numpy array, an int, or None."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+def _chk(status: int, where: str):
+    if status != LQCD_OK:
+        raise LqcdError(status, where)
+
+
+class Context:
+    """Owns one lqcd_ctx.  Methods carry the names of the C entry points minus the prefix."""
+
+    def __init__(self, dims, precision=64, recon=18, bc=(1, 1, 1, -1)):
+        p = lqcd_params()
+        p.dims[:] = [int(d) for d in dims]
+        p.precision, p.recon = int(precision), int(recon)
+        b = [complex(z) for z in bc]
+        p.bc_re[:] = [z.real for z in b]
+        p.bc_im[:] = [z.imag for z in b]
+        self._h = ctypes.c_void_p()
+        _chk(_lib().lqcd_create(ctypes.byref(self._h), ctypes.byref(p)), "lqcd_create")
+        self.dims, self.precision, self.recon = tuple(p.dims), p.precision, p.recon
+        self.Vh = self.dims[0] * self.dims[1] * self.dims[2] * self.dims[3] // 2
+
+    def __del__(self):
+        h, self._h = getattr(self, "_h", None), None
+        if h and _LIB is not None:
+            _LIB.lqcd_destroy(h)
+
+    # sizes
+    def spinor_bytes(self, half=True): return _lib().lqcd_spinor_bytes(self._h, int(half))
+    def gauge_bytes(self): return _lib().lqcd_gauge_bytes(self._h)
+    def workspace_bytes(self): return _lib().lqcd_workspace_bytes(self._h)
+    def host_workspace_bytes(self): return _lib().lqcd_host_workspace_bytes(self._h)
+
+    def set_block_threads(self, n):
+        _chk(_lib().lqcd_set_block_threads(self._h, int(n)), "lqcd_set_block_threads")
+
+    # layout conversion
+    def pack_gauge(self, native, canonical, stream=None):
+        _chk(_lib().lqcd_pack_gauge(self._h, _ptr(native), _ptr(canonical), _stream(stream)), "lqcd_pack_gauge")
+
+    def pack_spinor(self, native, canonical, parity, stream=None):
+        _chk(_lib().lqcd_pack_spinor(self._h, _ptr(native), _ptr(canonical), int(parity), _stream(stream)),
+             "lqcd_pack_spinor")
+
+    def unpack_spinor(self, canonical, native, parity, stream=None):
+        _chk(_lib().lqcd_unpack_spinor(self._h, _ptr(canonical), _ptr(native), int(parity), _stream(stream)),
+             "lqcd_unpack_spinor")
+
+    # hot path
+    def dslash_full(self, out, gauge, inp, stream=None):
+        _chk(_lib().lqcd_dslash_full(self._h, _ptr(out), _ptr(gauge), _ptr(inp), _stream(stream)), "lqcd_dslash_full")
+
+    def dslash_eo(self, out, gauge, inp, out_parity, stream=None):
+        _chk(_lib().lqcd_dslash_eo(self._h, _ptr(out), _ptr(gauge), _ptr(inp), int(out_parity), _stream(stream)),
+             "lqcd_dslash_eo")
+
+    def apply_M(self, out, gauge, inp, kappa, eo, workspace=None, stream=None):
+        _chk(_lib().lqcd_apply_M(self._h, _ptr(out), _ptr(gauge), _ptr(inp), float(kappa), int(eo),
+                                 _ptr(workspace), _stream(stream)), "lqcd_apply_M")
+
+    def dslash_eo_host(self, out_host, gauge_host, in_host, out_parity, workspace, stream=None):
+        _chk(_lib().lqcd_dslash_eo_host(self._h, _ptr(out_host), _ptr(gauge_host), _ptr(in_host), int(out_parity),
+                                        _ptr(workspace), _stream(stream)), "lqcd_dslash_eo_host")
+
+
+def launch_count() -> int:
+    return int(_lib().lqcd_launch_count())
+
+
+def real_dtype(precision):
+    import torch
+    return torch.float32 if precision == 32 else torch.float64
+
+
+def complex_dtype(precision):
+    import torch
+    return torch.complex64 if precision == 32 else torch.complex128

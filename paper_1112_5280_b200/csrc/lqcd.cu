@@ -1,0 +1,285 @@
+// lqcd.cu -- host side of the C ABI declared in include/lqcd.h: argument checks, template
+// dispatch (precision x recon x xpay x bc kind x block size) and kernel launches.
+// No field memory is allocated here and nothing synchronises except lqcd_dslash_eo_host.
+#include "../../include/lqcd.h"
+
+#include <atomic>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <new>
+
+#include "dslash_kernel.cuh"
+#include "pack_kernels.cuh"
+
+using namespace lqcd;
+
+struct lqcd_ctx {
+    lqcd_params p;
+    Geom g;
+    bool complex_bc;
+    int block;  // threads per block of the dslash kernel
+};
+
+namespace {
+
+std::atomic<unsigned long long> g_launches{0};
+thread_local char g_cuda_err[256] = "";
+
+lqcd_status cuda_fail(cudaError_t e) {
+    std::strncpy(g_cuda_err, cudaGetErrorString(e), sizeof(g_cuda_err) - 1);
+    return LQCD_ECUDA;
+}
+
+lqcd_status after_launch() {
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? LQCD_OK : cuda_fail(e);
+}
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+inline bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
+    const uintptr_t a0 = reinterpret_cast<uintptr_t>(a), b0 = reinterpret_cast<uintptr_t>(b);
+    return a0 < b0 + nb && b0 < a0 + na;
+}
+
+inline size_t elem(const lqcd_ctx* c) { return c->p.precision == 32 ? 4 : 8; }
+inline size_t half_bytes(const lqcd_ctx* c) { return (size_t)24 * c->g.Vh * elem(c); }
+inline size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
+
+template <typename R>
+BcPhases<R> make_bc(const lqcd_ctx* c) {
+    BcPhases<R> b;
+    for (int mu = 0; mu < 4; ++mu) {
+        b.re[mu] = (R)c->p.bc_re[mu];
+        b.im[mu] = (R)c->p.bc_im[mu];
+    }
+    return b;
+}
+
+template <typename R, int RECON, bool XPAY, bool CBC, int BLOCK>
+lqcd_status launch_block(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                         double a, int parity, cudaStream_t st) {
+    const dim3 grid((c->g.Vh + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
+    dslash_kernel<R, RECON, XPAY, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
+        (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, (R)a, c->g, parity < 0 ? 0 : parity, make_bc<R>(c));
+    return after_launch();
+}
+
+template <typename R, int RECON, bool XPAY, bool CBC>
+lqcd_status launch_cbc(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                       double a, int parity, cudaStream_t st) {
+    switch (c->block) {
+        case 64: return launch_block<R, RECON, XPAY, CBC, 64>(c, out, gauge, in, xin, a, parity, st);
+        case 128: return launch_block<R, RECON, XPAY, CBC, 128>(c, out, gauge, in, xin, a, parity, st);
+        case 256: return launch_block<R, RECON, XPAY, CBC, 256>(c, out, gauge, in, xin, a, parity, st);
+    }
+    return LQCD_EUNSUPPORTED;
+}
+
+template <typename R, int RECON>
+lqcd_status launch_recon(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                         double a, int parity, cudaStream_t st) {
+    if (xin) {
+        return c->complex_bc ? launch_cbc<R, RECON, true, true>(c, out, gauge, in, xin, a, parity, st)
+                             : launch_cbc<R, RECON, true, false>(c, out, gauge, in, xin, a, parity, st);
+    }
+    return c->complex_bc ? launch_cbc<R, RECON, false, true>(c, out, gauge, in, xin, a, parity, st)
+                         : launch_cbc<R, RECON, false, false>(c, out, gauge, in, xin, a, parity, st);
+}
+
+// out_p = H in (xin == NULL) or xin + a H in.  parity < 0: both parities, full fields.
+lqcd_status launch_dslash(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                          double a, int parity, cudaStream_t st) {
+    if (c->p.precision == 32) {
+        return c->p.recon == 12 ? launch_recon<float, 12>(c, out, gauge, in, xin, a, parity, st)
+                                : launch_recon<float, 18>(c, out, gauge, in, xin, a, parity, st);
+    }
+    return c->p.recon == 12 ? launch_recon<double, 12>(c, out, gauge, in, xin, a, parity, st)
+                            : launch_recon<double, 18>(c, out, gauge, in, xin, a, parity, st);
+}
+
+lqcd_status check_fields(const lqcd_ctx* c, const void* out, const void* gauge, const void* in, size_t nbytes) {
+    if (!c || !out || !gauge || !in) return LQCD_EINVAL;
+    if (!aligned16(out) || !aligned16(gauge) || !aligned16(in)) return LQCD_EALIGN;
+    if (overlaps(out, nbytes, in, nbytes)) return LQCD_EALIAS;
+    return LQCD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p) {
+    if (!ctx || !p) return LQCD_EINVAL;
+    if (p->precision != 32 && p->precision != 64) return LQCD_EINVAL;
+    if (p->recon != 12 && p->recon != 18) return LQCD_EINVAL;
+    double vol = 1;
+    bool cbc = false;
+    for (int mu = 0; mu < 4; ++mu) {
+        if (p->dims[mu] < 4 || (p->dims[mu] & 1)) return LQCD_EINVAL;
+        vol *= p->dims[mu];
+        const double n2 = p->bc_re[mu] * p->bc_re[mu] + p->bc_im[mu] * p->bc_im[mu];
+        if (!(std::fabs(n2 - 1.0) <= 1e-12)) return LQCD_EINVAL;
+        if (p->bc_im[mu] != 0.0) cbc = true;
+    }
+    // word indices (12 words x Vh per half spinor in fp64, 2*4*9*Vh link words) are kept below 2^31
+    if (vol / 2 * 72 >= 2147483648.0) return LQCD_EUNSUPPORTED;
+    lqcd_ctx* c = new (std::nothrow) lqcd_ctx;
+    if (!c) return LQCD_EINVAL;
+    c->p = *p;
+    Geom& g = c->g;
+    g.X = p->dims[0]; g.Y = p->dims[1]; g.Z = p->dims[2]; g.T = p->dims[3];
+    g.Xh = g.X / 2;
+    g.Vh = g.Xh * g.Y * g.Z * g.T;
+    g.sy = g.Xh; g.sz = g.Xh * g.Y; g.st = g.Xh * g.Y * g.Z;
+    c->complex_bc = cbc;
+    c->block = 128;
+    *ctx = c;
+    return LQCD_OK;
+}
+
+lqcd_status lqcd_destroy(lqcd_ctx* ctx) {
+    delete ctx;
+    return LQCD_OK;
+}
+
+size_t lqcd_spinor_bytes(const lqcd_ctx* c, int half) { return c ? half_bytes(c) * (half ? 1 : 2) : 0; }
+size_t lqcd_gauge_bytes(const lqcd_ctx* c) { return c ? (size_t)8 * c->p.recon * c->g.Vh * elem(c) : 0; }
+size_t lqcd_workspace_bytes(const lqcd_ctx* c) { return c ? half_bytes(c) : 0; }
+
+size_t lqcd_host_workspace_bytes(const lqcd_ctx* c) {
+    if (!c) return 0;
+    const size_t canon_gauge = (size_t)4 * 2 * c->g.Vh * 18 * elem(c);
+    return align256(lqcd_gauge_bytes(c)) + align256(canon_gauge) + 4 * align256(half_bytes(c));
+}
+
+lqcd_status lqcd_set_block_threads(lqcd_ctx* c, int b) {
+    if (!c) return LQCD_EINVAL;
+    if (b == 0) b = 128;
+    if (b != 64 && b != 128 && b != 256) return LQCD_EINVAL;
+    c->block = b;
+    return LQCD_OK;
+}
+
+lqcd_status lqcd_pack_gauge(const lqcd_ctx* c, void* native, const void* canon, void* stream) {
+    if (!c || !native || !canon) return LQCD_EINVAL;
+    if (!aligned16(native) || !aligned16(canon)) return LQCD_EALIGN;
+    const dim3 grid((c->g.Vh + 127) / 128, 4, 2);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (c->p.precision == 32) {
+        if (c->p.recon == 12) pack_gauge_kernel<float, 12><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);
+        else pack_gauge_kernel<float, 18><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);
+    } else {
+        if (c->p.recon == 12) pack_gauge_kernel<double, 12><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, c->g);
+        else pack_gauge_kernel<double, 18><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, c->g);
+    }
+    return after_launch();
+}
+
+static lqcd_status pack_unpack(const lqcd_ctx* c, void* dst, const void* src, int parity, void* stream, bool unpack) {
+    if (!c || !dst || !src) return LQCD_EINVAL;
+    if (parity < -1 || parity > 1) return LQCD_EINVAL;
+    if (!aligned16(dst) || !aligned16(src)) return LQCD_EALIGN;
+    const dim3 grid((c->g.Vh + 127) / 128, parity < 0 ? 2 : 1);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (c->p.precision == 32) {
+        if (unpack) pack_spinor_kernel<float, true><<<grid, 128, 0, st>>>((float*)dst, (const float*)src, c->g, parity);
+        else pack_spinor_kernel<float, false><<<grid, 128, 0, st>>>((float*)dst, (const float*)src, c->g, parity);
+    } else {
+        if (unpack) pack_spinor_kernel<double, true><<<grid, 128, 0, st>>>((double*)dst, (const double*)src, c->g, parity);
+        else pack_spinor_kernel<double, false><<<grid, 128, 0, st>>>((double*)dst, (const double*)src, c->g, parity);
+    }
+    return after_launch();
+}
+
+lqcd_status lqcd_pack_spinor(const lqcd_ctx* c, void* native, const void* canon, int parity, void* stream) {
+    return pack_unpack(c, native, canon, parity, stream, false);
+}
+
+lqcd_status lqcd_unpack_spinor(const lqcd_ctx* c, void* canon, const void* native, int parity, void* stream) {
+    return pack_unpack(c, canon, native, parity, stream, true);
+}
+
+lqcd_status lqcd_dslash_full(const lqcd_ctx* c, void* out, const void* gauge, const void* in, void* stream) {
+    lqcd_status s = check_fields(c, out, gauge, in, c ? 2 * half_bytes(c) : 0);
+    if (s != LQCD_OK) return s;
+    return launch_dslash(c, out, gauge, in, nullptr, 0.0, -1, (cudaStream_t)stream);
+}
+
+lqcd_status lqcd_dslash_eo(const lqcd_ctx* c, void* out, const void* gauge, const void* in, int out_parity,
+                           void* stream) {
+    if (out_parity != 0 && out_parity != 1) return LQCD_EINVAL;
+    lqcd_status s = check_fields(c, out, gauge, in, c ? half_bytes(c) : 0);
+    if (s != LQCD_OK) return s;
+    return launch_dslash(c, out, gauge, in, nullptr, 0.0, out_parity, (cudaStream_t)stream);
+}
+
+lqcd_status lqcd_apply_M(const lqcd_ctx* c, void* out, const void* gauge, const void* in, double kappa, int eo,
+                         void* workspace, void* stream) {
+    if (eo != 0 && eo != 1) return LQCD_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (eo == 0) {
+        lqcd_status s = check_fields(c, out, gauge, in, c ? 2 * half_bytes(c) : 0);
+        if (s != LQCD_OK) return s;
+        return launch_dslash(c, out, gauge, in, in, -kappa, -1, st);  // out = in - kappa H in
+    }
+    const size_t hb = c ? half_bytes(c) : 0;
+    lqcd_status s = check_fields(c, out, gauge, in, hb);
+    if (s != LQCD_OK) return s;
+    if (!workspace) return LQCD_EINVAL;
+    if (!aligned16(workspace)) return LQCD_EALIGN;
+    if (overlaps(workspace, hb, in, hb) || overlaps(workspace, hb, out, hb)) return LQCD_EALIAS;
+    s = launch_dslash(c, workspace, gauge, in, nullptr, 0.0, 1, st);  // tmp_o = H_oe in_e
+    if (s != LQCD_OK) return s;
+    return launch_dslash(c, out, gauge, workspace, in, -kappa * kappa, 0, st);  // out_e = in_e - k^2 H_eo tmp_o
+}
+
+lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* c, void* out_host, const void* gauge_host, const void* in_host,
+                                int out_parity, void* ws, void* stream) {
+    if (!c || !out_host || !in_host || !ws) return LQCD_EINVAL;
+    if (out_parity != 0 && out_parity != 1) return LQCD_EINVAL;
+    if (reinterpret_cast<uintptr_t>(ws) & 255u) return LQCD_EALIGN;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t hb = half_bytes(c);
+    const size_t canon_gauge = (size_t)4 * 2 * c->g.Vh * 18 * elem(c);
+    char* base = static_cast<char*>(ws);
+    char* g_nat = base;                 base += align256(lqcd_gauge_bytes(c));
+    char* g_can = base;                 base += align256(canon_gauge);
+    char* in_can = base;                base += align256(hb);
+    char* in_nat = base;                base += align256(hb);
+    char* out_nat = base;               base += align256(hb);
+    char* out_can = base;
+    cudaError_t e;
+    lqcd_status s;
+    if (gauge_host) {
+        if ((e = cudaMemcpyAsync(g_can, gauge_host, canon_gauge, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+        if ((s = lqcd_pack_gauge(c, g_nat, g_can, stream)) != LQCD_OK) return s;
+    }
+    if ((e = cudaMemcpyAsync(in_can, in_host, hb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if ((s = lqcd_pack_spinor(c, in_nat, in_can, 1 - out_parity, stream)) != LQCD_OK) return s;
+    if ((s = lqcd_dslash_eo(c, out_nat, g_nat, in_nat, out_parity, stream)) != LQCD_OK) return s;
+    if ((s = lqcd_unpack_spinor(c, out_can, out_nat, out_parity, stream)) != LQCD_OK) return s;
+    if ((e = cudaMemcpyAsync(out_host, out_can, hb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+    return LQCD_OK;
+}
+
+unsigned long long lqcd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+const char* lqcd_status_string(lqcd_status s) {
+    switch (s) {
+        case LQCD_OK: return "ok";
+        case LQCD_EINVAL: return "invalid argument";
+        case LQCD_EALIGN: return "device pointer not 16-byte aligned";
+        case LQCD_EALIAS: return "output overlaps an input";
+        case LQCD_EUNSUPPORTED: return "unsupported configuration";
+        case LQCD_ECUDA: return "CUDA error";
+    }
+    return "unknown status";
+}
+
+const char* lqcd_last_cuda_error(void) { return g_cuda_err; }
+
+}  // extern "C"
