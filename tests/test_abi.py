@@ -1,0 +1,61 @@
+"""CPU-side checks of the boundary: liblqcd.so loads, exports every symbol include/lqcd.h
+declares, and the host logic that needs no GPU (parameter validation, size queries)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_1112_5280_b200 as L
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "lqcd.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(lqcd_[a-zA-Z_0-9]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_1112_5280_b200 import _build
+    _build.build()
+    lib = ctypes.CDLL(_build.LIB)
+    names = _declared()
+    assert len(names) >= 15
+    for n in names:
+        assert hasattr(lib, n), n
+    assert sorted(L.EXPORTS) == names
+
+
+def test_create_validation_and_sizes():
+    c = L.Context((32, 32, 32, 64), 32, 12)
+    Vh = 32 * 32 * 32 * 64 // 2
+    assert c.Vh == Vh
+    assert c.spinor_bytes(True) == Vh * 24 * 4
+    assert c.spinor_bytes(False) == Vh * 48 * 4
+    assert c.gauge_bytes() == 8 * 12 * Vh * 4
+    assert c.workspace_bytes() == Vh * 24 * 4
+    c = L.Context((4, 4, 4, 4), 64, 18)
+    assert c.gauge_bytes() == 8 * 18 * 128 * 8
+    assert c.host_workspace_bytes() >= c.gauge_bytes() + 4 * 256 * 18 * 8 + 4 * c.spinor_bytes(True)
+    for bad in [dict(dims=(4, 4, 3, 4)), dict(dims=(2, 4, 4, 4)), dict(precision=16), dict(recon=8),
+                dict(bc=(1, 1, 1, 0.5))]:
+        kw = dict(dims=(4, 4, 4, 4), precision=64, recon=18, bc=(1, 1, 1, -1))
+        kw.update(bad)
+        with pytest.raises(L.LqcdError) as e:
+            L.Context(**kw)
+        assert e.value.status == L.LQCD_EINVAL
+    c.set_block_threads(256)
+    with pytest.raises(L.LqcdError):
+        c.set_block_threads(100)
+
+
+def test_null_pointers_rejected_without_gpu():
+    c = L.Context((4, 4, 4, 4), 64, 18)
+    lib = L._lib()
+    assert lib.lqcd_dslash_eo(c._h, None, None, None, 0, None) == L.LQCD_EINVAL
+    assert lib.lqcd_dslash_full(None, None, None, None, None) == L.LQCD_EINVAL
+    assert lib.lqcd_apply_M(c._h, None, None, None, 0.1, 2, None, None) == L.LQCD_EINVAL
+    assert lib.lqcd_spinor_bytes(None, 1) == 0
+    assert lib.lqcd_status_string(L.LQCD_EALIAS).decode() == "output overlaps an input"

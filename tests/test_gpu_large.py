@@ -1,0 +1,102 @@
+"""GPU parity at BASELINE.json's full sizes (configs 4 and 5), in the launch configuration
+bench.py times: the oracle computes sampled output sites one by one (oracle.dslash_sites /
+apply_M_sites) and the CUDA result is compared there; plus properties that hold at any size.
+"""
+import numpy as np
+import pytest
+
+import lattice_inputs as li
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL = {64: 1e-12, 32: 1e-5}
+
+
+def sample_sites(dims, parity, n, seed):
+    """n random sites of the given parity plus the corners/faces where the wrap logic lives."""
+    X, Y, Z, T = dims
+    rng = np.random.default_rng(seed)
+    c = np.stack([rng.integers(0, L, size=4 * n) for L in dims], axis=1)
+    edge = [[a, b, cc, d] for a in (0, 1, X - 2, X - 1) for b in (0, Y - 1) for cc in (0, Z - 1) for d in (0, 1, T - 1)]
+    c = np.concatenate([np.array(edge), c])
+    c = c[(c.sum(axis=1) & 1) == parity]
+    return c[: n + len(edge)]
+
+
+def cb_index(dims, coords):
+    X, Y, Z, T = dims
+    lex = coords[:, 0] + X * (coords[:, 1] + Y * (coords[:, 2] + Z * coords[:, 3]))
+    return lex >> 1
+
+
+@pytest.fixture(scope="module")
+def cfg4():
+    c = li.CONFIGS[4]
+    U = li.links_for_config(4)
+    psi = li.gaussian_spinor(c["dims"])
+    return c, U, psi
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_config4_eo_recon12_sampled(cfg4, precision):
+    import gpu_harness as H
+    c, U64, psi64 = cfg4
+    dims, bc = c["dims"], c["bc"]
+    U = U64.astype(H.cdtype(precision))
+    psi = psi64.astype(H.cdtype(precision))
+    g = H.Gpu(dims, precision, 12, bc, U)
+    for out_parity in (0, 1):
+        got = g.dslash_eo(H.half_of(psi, dims, 1 - out_parity), out_parity)
+        sites = sample_sites(dims, out_parity, 4096, seed=40 + out_parity)
+        ref = oracle.dslash_sites(U, psi, dims, bc, sites)
+        assert H.rel_l2(got[cb_index(dims, sites)], ref) <= TOL[precision]
+        assert np.isfinite(got.view(np.float32 if precision == 32 else np.float64)).all()
+    # host-buffer entry point (what bench.py's e2e leg times) gives the same result bit for bit
+    import torch
+    ws = torch.empty(g.ctx.host_workspace_bytes(), dtype=torch.uint8, device="cuda:0")
+    in_h = torch.from_numpy(H.half_of(psi, dims, 1)).pin_memory()
+    U_h = torch.from_numpy(np.ascontiguousarray(U)).pin_memory()
+    out_h = torch.empty_like(in_h).pin_memory()
+    g.ctx.dslash_eo_host(out_h, U_h, in_h, 0, ws)
+    dev = g.dslash_eo(H.half_of(psi, dims, 1), 0)
+    assert np.array_equal(out_h.numpy(), dev)
+
+
+def test_config4_full_field_fp32_vs_oracle(cfg4):
+    """Whole-field comparison at the headline size (the oracle needs a few seconds here)."""
+    import gpu_harness as H
+    c, U64, psi64 = cfg4
+    dims, bc = c["dims"], c["bc"]
+    U = U64.astype(np.complex64)
+    psi = psi64.astype(np.complex64)
+    g = H.Gpu(dims, 32, 12, bc, U)
+    ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, 0), dims, 0)
+    assert H.rel_l2(g.dslash_eo(H.half_of(psi, dims, 1), 0), ref) <= TOL[32]
+
+
+@pytest.mark.parametrize("recon", [12, 18])
+def test_config5_chain_per_step_parity(recon):
+    """Config 5 (reading A16): x_{k+1} = M x_k chained 100 times in fp32; per-step parity at
+    k in {1, 50, 100}: the oracle is fed the GPU's own x_k and compared with x_{k+1} at sampled sites."""
+    import torch
+    import gpu_harness as H
+    c = li.CONFIGS[5]
+    dims, bc, kappa = c["dims"], c["bc"], c["kappa"]
+    U = li.links_for_config(5, dtype=np.complex64)
+    psi = li.gaussian_spinor(dims, dtype=np.complex64)
+    g = H.Gpu(dims, 32, recon, bc, U)
+    x = g.to_native(H.half_of(psi, dims, 0), 0)
+    y, ws = g.buf(), g.buf()
+    sites = sample_sites(dims, 0, 1024, seed=50)
+    idx = cb_index(dims, sites)
+    for k in range(1, 101):
+        g.ctx.apply_M(y, g.gauge, x, kappa, 1, ws)
+        if k in (1, 50, 100):
+            xk = H.scatter_half(g.from_native(x, 0), dims, 0)
+            got = g.from_native(y, 0)
+            assert np.isfinite(got.view(np.float32)).all()
+            ref = oracle.apply_M_sites(U, xk, dims, bc, kappa, 1, sites)
+            assert H.rel_l2(got[idx], ref) <= TOL[32], k
+        x, y = y, x
+    torch.cuda.synchronize()

@@ -1,0 +1,173 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are BASELINE.json north_star's: relative L2 error
+<= 1e-12 (fp64), <= 1e-5 (fp32)  (error norm: SURVEY.md A15).
+"""
+import numpy as np
+import pytest
+
+import lattice_inputs as li
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL = {64: 1e-12, 32: 1e-5}
+
+
+def _inputs(cfg_id, precision):
+    from gpu_harness import cdtype
+    c = li.CONFIGS[cfg_id]
+    cd = cdtype(precision)
+    # fp32 runs: inputs rounded to fp32 once, the oracle promotes those values (reading A14)
+    U = li.links_for_config(cfg_id).astype(cd)
+    psi = li.gaussian_spinor(c["dims"]).astype(cd)
+    return c, U, psi
+
+
+@pytest.fixture(scope="module")
+def H():
+    import gpu_harness
+    return gpu_harness
+
+
+# ------------------------------------------------------------------ config 1: 4^4 fp64 full
+@pytest.mark.parametrize("recon", [18, 12])
+def test_config1_full_fp64(H, recon):
+    c, U, psi = _inputs(1, 64)
+    g = H.Gpu(c["dims"], 64, recon, c["bc"], U)
+    ref = oracle.dslash_full(U, psi, c["dims"], c["bc"])
+    assert H.rel_l2(g.dslash_full(psi), ref) <= TOL[64]
+    refM = oracle.apply_M(U, psi, c["dims"], c["bc"], c["kappa"], 0)
+    assert H.rel_l2(g.apply_M(psi, c["kappa"], 0), refM) <= TOL[64]
+
+
+def test_config1_free_field_plane_wave(H):
+    """Unit links: M psi = [(1 - 2k sum cos p) + 2ik sum gamma_mu sin p_mu] psi sitewise (pin P1 on the GPU)."""
+    c = li.CONFIGS[1]
+    dims, bc, kappa = c["dims"], c["bc"], c["kappa"]
+    U = li.unit_links(dims)
+    g = H.Gpu(dims, 64, 18, bc, U)
+    rng = np.random.default_rng(5)
+    for n in [(0, 0, 0, 0), (1, 0, 0, 0), (1, 2, 3, 1), (2, 2, 2, 2), (3, 1, 0, 2)]:
+        chi = rng.standard_normal((4, 3)) + 1j * rng.standard_normal((4, 3))
+        psi, p = li.plane_wave(dims, n, bc, chi)
+        m = (1 - 2 * kappa * np.cos(p).sum()) * np.eye(4, dtype=complex)
+        for mu in range(4):
+            m = m + 2j * kappa * np.sin(p[mu]) * oracle.gamma(mu)
+        expect = np.einsum("st,...ta->...sa", m, psi)
+        assert H.rel_l2(g.apply_M(psi, kappa, 0), expect) <= TOL[64]
+
+
+# ------------------------------------------------------------------ config 2: 8^3x16 fp64 eo
+@pytest.mark.parametrize("recon", [18, 12])
+def test_config2_eo_fp64(H, recon):
+    c, U, psi = _inputs(2, 64)
+    dims, bc = c["dims"], c["bc"]
+    g = H.Gpu(dims, 64, recon, bc, U)
+    for out_parity in (0, 1):
+        ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, out_parity), dims, out_parity)
+        got = g.dslash_eo(H.half_of(psi, dims, 1 - out_parity), out_parity)
+        assert H.rel_l2(got, ref) <= TOL[64]
+    # even-odd pieces reassemble the full operator (pin P4 on the GPU)
+    full = g.dslash_full(psi)
+    assert H.rel_l2(full, oracle.dslash_full(U, psi, dims, bc)) <= TOL[64]
+    refM = H.half_of(oracle.apply_M(U, psi, dims, bc, c["kappa"], 1), dims, 0)
+    assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), c["kappa"], 1), refM) <= TOL[64]
+
+
+def test_config2_gamma5_hermiticity_and_covariance(H):
+    """P3 and P5 evaluated on GPU outputs (properties that hold at any size)."""
+    c, U, psi = _inputs(2, 64)
+    dims, bc = c["dims"], c["bc"]
+    g = H.Gpu(dims, 64, 12, bc, U)
+    phi = li.gaussian_spinor(dims, seed=11)
+    g5 = np.array([1, 1, -1, -1])[:, None]
+    lhs = np.vdot(phi, g.dslash_full(psi))
+    rhs = np.vdot(g5 * g.dslash_full(g5 * phi), psi)
+    assert abs(lhs - rhs) / abs(lhs) <= 1e-12
+    gx = li.random_su3_field(dims, seed=3)
+    Ug = np.empty_like(U)
+    for mu in range(4):
+        gshift = np.roll(gx, -1, axis=3 - mu)
+        Ug[mu] = gx @ U[mu] @ np.conj(np.swapaxes(gshift, -1, -2))
+    g2 = H.Gpu(dims, 64, 12, bc, Ug)
+    psig = np.einsum("...ab,...sb->...sa", gx, psi)
+    expect = np.einsum("...ab,...sb->...sa", gx, g.dslash_full(psi))
+    assert H.rel_l2(g2.dslash_full(psig), expect) <= 1e-12
+
+
+# ------------------------------------------------------------------ config 3: 16^3x32 full, fp32 + fp64
+@pytest.mark.parametrize("precision,recon", [(64, 18), (64, 12), (32, 18), (32, 12)])
+def test_config3_full(H, precision, recon):
+    c, U, psi = _inputs(3, precision)
+    dims, bc = c["dims"], c["bc"]
+    g = H.Gpu(dims, precision, recon, bc, U)
+    assert H.rel_l2(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc)) <= TOL[precision]
+    refM = oracle.apply_M(U, psi, dims, bc, c["kappa"], 0)
+    assert H.rel_l2(g.apply_M(psi, c["kappa"], 0), refM) <= TOL[precision]
+
+
+# ------------------------------------------------------------------ edge cases
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_ragged_anisotropic_complex_bc(H, precision, recon):
+    """Vh = 960 is not a multiple of the block size; all extents differ; general U(1) phases."""
+    from gpu_harness import cdtype
+    dims = (4, 6, 8, 10)
+    bc = np.exp(1j * np.array([0.3, -1.1, 2.0, np.pi]))
+    U = li.random_su3_links(dims, seed=21).astype(cdtype(precision))
+    psi = li.gaussian_spinor(dims, seed=22).astype(cdtype(precision))
+    g = H.Gpu(dims, precision, recon, bc, U)
+    for blk in (64, 128, 256):
+        g.ctx.set_block_threads(blk)
+        assert H.rel_l2(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc)) <= TOL[precision]
+        for op in (0, 1):
+            ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, op), dims, op)
+            assert H.rel_l2(g.dslash_eo(H.half_of(psi, dims, 1 - op), op), ref) <= TOL[precision]
+    refM = H.half_of(oracle.apply_M(U, psi, dims, bc, 0.13, 1), dims, 0)
+    assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), 0.13, 1), refM) <= TOL[precision]
+
+
+def test_minimum_extent_and_all_periodic(H):
+    dims = (4, 4, 4, 4)
+    U = li.random_su3_links(dims, seed=31)
+    psi = li.gaussian_spinor(dims, seed=32)
+    for bc in [(1, 1, 1, 1), (-1, -1, -1, -1)]:
+        g = H.Gpu(dims, 64, 12, bc, U)
+        assert H.rel_l2(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc)) <= TOL[64]
+
+
+def test_pack_unpack_roundtrip_bit_exact(H):
+    dims = (4, 6, 8, 10)
+    U = li.random_su3_links(dims, seed=21)
+    psi = li.gaussian_spinor(dims, seed=22)
+    for precision in (64, 32):
+        g = H.Gpu(dims, precision, 18, (1, 1, 1, -1), U)
+        p = psi.astype(H.cdtype(precision))
+        assert np.array_equal(g.from_native(g.to_native(p, -1), -1), p)
+        for par in (0, 1):
+            h = H.half_of(p, dims, par)
+            assert np.array_equal(g.from_native(g.to_native(h, par), par), h)
+
+
+def test_error_codes(H):
+    import torch
+    import paper_1112_5280_b200 as L
+    dims = (4, 4, 4, 4)
+    g = H.Gpu(dims, 64, 18, (1, 1, 1, -1), li.unit_links(dims))
+    a, b = g.buf(), g.buf()
+    with pytest.raises(L.LqcdError) as e:
+        g.ctx.dslash_eo(a, g.gauge, a, 0)
+    assert e.value.status == L.LQCD_EALIAS
+    with pytest.raises(L.LqcdError) as e:
+        g.ctx.dslash_eo(a, g.gauge, b, 2)
+    assert e.value.status == L.LQCD_EINVAL
+    with pytest.raises(L.LqcdError) as e:
+        g.ctx.dslash_eo(a.data_ptr() + 8, g.gauge, b, 0)
+    assert e.value.status == L.LQCD_EALIGN
+    with pytest.raises(L.LqcdError) as e:
+        g.ctx.apply_M(a, g.gauge, b, 0.1, 1, None)
+    assert e.value.status == L.LQCD_EINVAL
+    with pytest.raises(L.LqcdError) as e:
+        g.ctx.apply_M(a, g.gauge, b, 0.1, 1, b)
+    assert e.value.status == L.LQCD_EALIAS
+    torch.cuda.synchronize()
