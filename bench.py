@@ -1,0 +1,471 @@
+#!/usr/bin/env python
+"""bench.py -- Wilson dslash benchmark on B200 (BASELINE.json metric: dslash GFLOP/s at 1320 flop/site
+and achieved HBM GB/s vs roofline at 32^3x64).
+
+    python bench.py --gpus 1 --steps K --warmup W            # this repo's CUDA path (default)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle on the host cores
+
+Workload (config.workload): BASELINE.json configs[3] = SURVEY.md sec. 8(d) config 4, the headline
+bandwidth case: 32^3x64, even-odd dslash, 12-real links, random SU(3) links (seed 1), Gaussian
+spinors (seed 2), antiperiodic in t.  Primary line fp32; the fp64 case and the config-5 style
+M-chain are reported in the same JSON line under "fp64" and "chain".
+
+A step = one pass of the hot path (K1..L6 of SURVEY.md sec. 8(a)) over one batch of NBUF = 4
+half-lattice spinors: NBUF launches of lqcd_dslash_eo, alternating out_parity 0,1 (H_eo, H_oe),
+each reading its own input buffer and writing its own output buffer.  Rotating buffers keeps the
+spinor working set (NBUF x 2 x 100/201 MB) above the 126 MB L2 so no launch finds its input
+resident from the previous one; the 403/805 MB link field is streamed once per launch.
+
+Multi-GPU: the path does not shard in this build ("replicas only"): --gpus N runs N
+independent replicas, one process per GPU, no data-path collective; value = N replicas' sites / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FLOP_PER_SITE = 1320                  # BASELINE.json convention: 8 x (12 + 132) + 7 x 24
+REALS_PER_SITE = {12: 144, 18: 192}   # compulsory eo model: 24 in + 24 out + 8 links
+NBUF = 4
+METRIC = "dslash GFLOP/s (1320 flop/site), 32^3x64 even-odd recon-12"
+FALLBACK_HBM_GBS = 6650.0             # /opt/skills/guides/B200_PROFILING.md fallback
+NOMINAL_HBM_GBS = 8000.0              # north_star's "~8 TB/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=500)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="lattice_inputs.CONFIGS id of the main workload")
+    ap.add_argument("--precision", type=int, default=32, choices=[32, 64], help="precision of the primary line")
+    ap.add_argument("--recon", type=int, default=12, choices=[12, 18])
+    ap.add_argument("--block", type=int, default=0, help="dslash block size override (tuning)")
+    ap.add_argument("--chain", action="store_true", help="also time config 5: apply_M(eo=1) x100 chained at 48^3x96")
+    ap.add_argument("--no-extras", action="store_true", help="skip the fp64 / chain / e2e / cpu legs (profiling runs)")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, device copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(precision, recon):
+    """dram bytes per launch of the dslash kernel from the committed ncu --set full summary, or None."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    try:
+        with open(path) as f:
+            for line in f:
+                p = [x.strip() for x in line.split(",")]
+                if len(p) >= 4 and p[0] == "config4" and p[1] == f"fp{precision}" and p[2] == f"recon{recon}":
+                    return float(p[3])
+    except OSError:
+        pass
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms while the kernels run."""
+    Q = ("clocks.sm,clocks.max.sm,utilization.gpu,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
+    def __init__(self, index):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)
+        self.proc.terminate()
+        self.thr.join(timeout=2)
+        sm, smax, reasons, n = [], None, set(), 0
+        for ts, line in self.rows:
+            if not (t0 <= ts <= t1 + 0.06):
+                continue
+            p = [x.strip() for x in line.split(",")]
+            try:
+                clk, mx, util = float(p[0]), float(p[1]), float(p[2])
+            except (ValueError, IndexError):
+                continue
+            n += 1
+            smax = mx
+            if util >= 50 or not sm:
+                sm.append(clk)
+            for name, v in zip(self.NAMES, p[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": n}
+
+
+# ------------------------------------------------------------------------------------------------
+# this repo's arm
+# ------------------------------------------------------------------------------------------------
+class Workload:
+    """Seeded inputs of one config on the device in native layout, plus pinned host copies."""
+
+    def __init__(self, cfg_id, precision, recon, dev, block=0, nbuf=NBUF, keep_host=True, in_parity=None):
+        import numpy as np
+        import torch
+        import lattice_inputs as li
+        import paper_1112_5280_b200 as L
+        self.L, self.torch = L, torch
+        c = li.CONFIGS[cfg_id]
+        self.cfg_id, self.dims, self.bc, self.kappa = cfg_id, c["dims"], c["bc"], c["kappa"]
+        self.precision, self.recon, self.dev, self.nbuf = precision, recon, dev, nbuf
+        cd = np.complex64 if precision == 32 else np.complex128
+        self.ctx = L.Context(self.dims, precision, recon, self.bc)
+        if block:
+            self.ctx.set_block_threads(block)
+        self.Vh = self.ctx.Vh
+        U = li.links_for_config(cfg_id, dtype=cd)
+        self.U_host = torch.from_numpy(U).pin_memory() if keep_host else None
+        self.gauge = torch.empty(self.ctx.gauge_bytes(), dtype=torch.uint8, device=dev)
+        Ud = torch.from_numpy(U).to(dev)
+        self.ctx.pack_gauge(self.gauge, Ud)
+        torch.cuda.synchronize(dev)
+        del Ud, U
+        mask = [li.parity_mask(self.dims, p).ravel() for p in (0, 1)]
+        self.inp, self.out, self.in_host = [], [], []
+        for b in range(nbuf):
+            out_parity = (b & 1) if in_parity is None else 1 - in_parity
+            psi = li.gaussian_spinor(self.dims, seed=li.SPINOR_SEED + b, dtype=cd)
+            half = np.ascontiguousarray(psi.reshape(-1, 4, 3)[mask[1 - out_parity]])
+            h = torch.from_numpy(half).pin_memory()
+            n = torch.empty(self.ctx.spinor_bytes(True), dtype=torch.uint8, device=dev)
+            self.ctx.pack_spinor(n, h.to(dev), 1 - out_parity)
+            self.inp.append(n)
+            self.out.append(torch.empty_like(n))
+            if keep_host:
+                self.in_host.append(h)
+        torch.cuda.synchronize(dev)
+
+    def step(self):
+        for b in range(self.nbuf):
+            self.ctx.dslash_eo(self.out[b], self.gauge, self.inp[b], b & 1)
+
+    def sites_per_step(self):
+        return self.nbuf * self.Vh
+
+    def bytes_per_launch(self):
+        return REALS_PER_SITE[self.recon] * (self.precision // 8) * self.Vh
+
+
+def timed_steps(torch, dist, fn, steps, warmup):
+    """W untimed steps, then K steps between two CUDA events on the launching (current) stream,
+    barrier + synchronize on both sides; returns max-over-ranks milliseconds for the K steps."""
+    for _ in range(warmup):
+        fn()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    ms = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return ms
+
+
+def kernel_leg(torch, dist, w, steps, warmup, world):
+    """Device-resident timing of one Workload: returns the numbers of one precision/recon case."""
+    L = w.L
+    n0 = L.launch_count()
+    ms = timed_steps(torch, dist, w.step, steps, warmup)
+    launches = (L.launch_count() - n0) - warmup * w.nbuf
+    ms_step = ms / steps
+    t_launch = ms_step / w.nbuf * 1e-3
+    return {
+        "ms_per_step": ms_step,
+        "us_per_launch": t_launch * 1e6,
+        "gflops": world * w.sites_per_step() * FLOP_PER_SITE / (ms_step * 1e-3) / 1e9,
+        "gbs": w.bytes_per_launch() / t_launch / 1e9,
+        "launches": launches,
+    }
+
+
+def e2e_leg(torch, w, steps, world):
+    """Same metric through the host-buffer entry point lqcd_dslash_eo_host: pinned canonical half
+    spinor in (H2D), pack, dslash, unpack, canonical half spinor out (D2H) inside the timed region.
+    The link field is uploaded once before (it is constant across applications, like weights)."""
+    ctx = w.ctx
+    ws = torch.empty(ctx.host_workspace_bytes(), dtype=torch.uint8, device=w.dev)
+    out_h = [torch.empty_like(h).pin_memory() for h in w.in_host]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # gauge upload + pack + one application, timed separately (3 repetitions, best)
+    tg = []
+    for _ in range(3):
+        torch.cuda.synchronize()
+        e0.record()
+        ctx.dslash_eo_host(out_h[0], w.U_host, w.in_host[0], 0, ws)
+        e1.record()
+        torch.cuda.synchronize()
+        tg.append(e0.elapsed_time(e1))
+    for b in range(w.nbuf):  # warm-up
+        ctx.dslash_eo_host(out_h[b], None, w.in_host[b], b & 1, ws)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(steps):
+        for b in range(w.nbuf):
+            ctx.dslash_eo_host(out_h[b], None, w.in_host[b], b & 1, ws)
+    e1.record()
+    torch.cuda.synchronize()
+    wall = (time.perf_counter() - t0) * 1e3
+    ms = max(e0.elapsed_time(e1), wall) / steps
+    hb = w.in_host[0].numel() * w.in_host[0].element_size()
+    return {
+        "value": world * w.sites_per_step() * FLOP_PER_SITE / (ms * 1e-3) / 1e9,
+        "unit": "GFLOP/s",
+        "h2d_bytes_per_step": hb * w.nbuf,
+        "d2h_bytes_per_step": hb * w.nbuf,
+        "ms_per_step": ms,
+        "steps": steps,
+        "gauge": "resident (uploaded and packed once before the timed region)",
+        "ms_one_application_with_gauge_upload": min(tg),
+        "gauge_h2d_bytes": w.U_host.numel() * w.U_host.element_size(),
+    }
+
+
+def chain_leg(torch, cfg_id, precision, recon, dev, napply=100, reps=3):
+    """Config 5 (reading A16): x_{k+1} = M x_k, M = 1 - kappa^2 H_eo H_oe, `napply` times back to back,
+    ping-pong buffers, timed as one block."""
+    w = Workload(cfg_id, precision, recon, dev, nbuf=1, keep_host=False, in_parity=0)  # even half spinor
+    x, y = w.inp[0], w.out[0]
+    ws = torch.empty_like(x)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    best = None
+    for _ in range(reps + 1):
+        a, b = x.clone(), y
+        torch.cuda.synchronize()
+        e0.record()
+        for _k in range(napply):
+            w.ctx.apply_M(b, w.gauge, a, w.kappa, 1, ws)
+            a, b = b, a
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None else min(best, ms)
+    reals = REALS_PER_SITE[recon] * 2 + 24  # pass 1 + pass 2 with the xpay read
+    nbytes = reals * (precision // 8) * w.Vh
+    finite = bool(torch.isfinite(a.view(torch.float32 if precision == 32 else torch.float64)).all().item())
+    return {
+        "workload": f"config {cfg_id}: {'x'.join(map(str, w.dims))} fp{precision} recon-{recon} apply_M(eo=1) x{napply} chained",
+        "ms_per_chain": best, "ms_per_application": best / napply,
+        "gflops": 2 * FLOP_PER_SITE * w.Vh * napply / (best * 1e-3) / 1e9,
+        "gbs": nbytes * napply / (best * 1e-3) / 1e9,
+        "bytes_per_application": nbytes, "finite": finite,
+    }
+
+
+def cpu_baseline_leg(cfg_id, precision):
+    """The oracle as it stands on the host cores: full-lattice dslash_eo of the same workload,
+    one warm-up then best of 3 (about 2-5 s of CPU work on 8+ cores)."""
+    import numpy as np
+    import lattice_inputs as li
+    import oracle
+    c = li.CONFIGS[cfg_id]
+    cd = np.complex64 if precision == 32 else np.complex128
+    U = li.links_for_config(cfg_id, dtype=cd)
+    psi = li.gaussian_spinor(c["dims"], dtype=cd)
+    Vh = int(np.prod(c["dims"])) // 2
+    oracle.dslash_eo(U, psi, c["dims"], c["bc"], 0)
+    best = None
+    for _ in range(3):
+        t0 = time.perf_counter()
+        oracle.dslash_eo(U, psi, c["dims"], c["bc"], 0)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return {"value": Vh * FLOP_PER_SITE / best / 1e9, "unit": "GFLOP/s", "cores": oracle.num_threads(),
+            "kind": "oracle",
+            "sample": f"config {cfg_id}: one full oracle.dslash_eo (V/2 = {Vh} output sites, fp64 arithmetic on "
+                      f"fp{precision} inputs), best of 3 after one warm-up, {best * 1e3:.0f} ms"}
+
+
+def run_b200(args):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA path is the only implementation; no CPU fallback)")
+    import __graft_entry__ as ge
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist_.init_process_group("nccl", device_id=dev)
+        dist = dist_
+    if rank == 0:
+        ge.build()
+    if dist is not None:
+        dist.barrier()
+    import paper_1112_5280_b200 as L
+    L._lib()
+    peak, peak_src = measured_peaks()
+
+    w = Workload(args.config, args.precision, args.recon, dev, args.block)
+    sampler = ClockSampler(local) if rank == 0 else None
+    t0 = time.time()
+    main = kernel_leg(torch, dist, w, args.steps, args.warmup, world)
+    # keep the same launches running until nvidia-smi has seen >= 1.5 s of them (clocks under load)
+    while time.time() - t0 < 1.5:
+        for _ in range(20):
+            w.step()
+        torch.cuda.synchronize()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1) if sampler else None
+    if clocks is not None:
+        clocks["window"] = "warm-up + timed region + untimed continuation of the same launches to >= 1.5 s"
+
+    line = {
+        "metric": METRIC, "value": main["gflops"], "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": f"f{args.precision}", "data": "synthetic",
+        "config": {
+            "workload": f"config {args.config}: {'x'.join(map(str, w.dims))} even-odd dslash, recon-{args.recon}, "
+                        f"fp{args.precision}, random SU(3) links seed 1, Gaussian spinors seed 2.., bc (+,+,+,-)",
+            "step": f"{w.nbuf} lqcd_dslash_eo launches (out_parity 0,1,0,1) over {w.nbuf} distinct in/out half spinors",
+            "sites_per_step": w.sites_per_step(),
+            "l2": "inputs larger than L2: links %.0f MB streamed per launch + %.0f MB of rotating spinor buffers; no flush"
+                  % (w.ctx.gauge_bytes() / 1e6, 2 * w.nbuf * w.ctx.spinor_bytes(True) / 1e6),
+            "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
+        },
+        "gpu_launches": main["launches"],
+        "achieved_gbs": main["gbs"],
+        "us_per_launch": main["us_per_launch"],
+        "clocks": clocks,
+        "roofline": {
+            "bound": "hbm", "achieved": main["gbs"], "peak": peak, "unit": "GB/s", "frac": main["gbs"] / peak,
+            "traffic": ncu_traffic(args.precision, args.recon), "peak_source": peak_src,
+            "kernel": f"dslash_kernel<fp{args.precision}, recon {args.recon}>",
+            "model": f"compulsory {REALS_PER_SITE[args.recon]} reals/site x {args.precision // 8} B x V/2 = {w.bytes_per_launch()} B per launch",
+            "frac_of_nominal_8TBs": main["gbs"] / NOMINAL_HBM_GBS,
+        },
+    }
+
+    if not args.no_extras and rank == 0:
+        line["e2e"] = e2e_leg(torch, w, max(1, min(args.steps, 10)), 1)
+    del w
+    torch.cuda.empty_cache()
+    if not args.no_extras:
+        other = 64 if args.precision == 32 else 32
+        w2 = Workload(args.config, other, args.recon, dev, args.block, keep_host=False)
+        r2 = kernel_leg(torch, dist, w2, max(1, args.steps // 2), args.warmup, world)
+        line[f"fp{other}"] = {"gflops": r2["gflops"], "achieved_gbs": r2["gbs"], "frac": r2["gbs"] / peak,
+                              "frac_of_nominal_8TBs": r2["gbs"] / NOMINAL_HBM_GBS, "us_per_launch": r2["us_per_launch"],
+                              "traffic": ncu_traffic(other, args.recon)}
+        del w2
+        torch.cuda.empty_cache()
+        if rank == 0:
+            if args.chain:  # config 5; opt-in: generating its 3 GB A11 link field takes minutes of host time
+                line["chain"] = [chain_leg(torch, 5, 32, rc, dev) for rc in (12, 18)]
+            line["cpu_baseline"] = cpu_baseline_leg(args.config, args.precision)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle on the host cores (this tier has no reference implementation)
+# ------------------------------------------------------------------------------------------------
+def run_reference(args):
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import numpy as np
+    import lattice_inputs as li
+    import oracle
+    oracle.build()
+    c = li.CONFIGS[args.config]
+    dims, bc = c["dims"], c["bc"]
+    cd = np.complex64 if args.precision == 32 else np.complex128
+    U = li.links_for_config(args.config, dtype=cd)
+    psi = li.gaussian_spinor(dims, dtype=cd)
+    X, Y, Z, T = dims
+    V = X * Y * Z * T
+    # a step = oracle.dslash_sites on a bounded sample of the workload's output sites (every `stride`-th
+    # lexicographic site), sized from one calibration call so K + W steps end within ~2 minutes
+    def sites_for(n):
+        lex = np.linspace(0, V - 1, n).astype(np.int64)
+        return np.stack([lex % X, (lex // X) % Y, (lex // (X * Y)) % Z, lex // (X * Y * Z)], axis=1).astype(np.int32)
+    probe = sites_for(65536)
+    oracle.dslash_sites(U, psi, dims, bc, probe)
+    t0 = time.perf_counter()
+    oracle.dslash_sites(U, psi, dims, bc, probe)
+    per_site = (time.perf_counter() - t0) / len(probe)
+    budget = 120.0 / max(1, args.steps + args.warmup)
+    n = int(max(1024, min(V // 2, budget / per_site)))
+    sites = sites_for(n)
+    for _ in range(args.warmup):
+        oracle.dslash_sites(U, psi, dims, bc, sites)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.dslash_sites(U, psi, dims, bc, sites)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = n * FLOP_PER_SITE / dt / 1e9
+    sample = f"{n} output sites of config {args.config} per step via oracle.dslash_sites (fp64 arithmetic on fp{args.precision} inputs)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "GFLOP/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config {args.config}: {'x'.join(map(str, dims))} even-odd dslash (CPU oracle, host cores)",
+                   "sample": sample},
+        "gpu_launches": 0,
+        "cpu_baseline": {"value": val, "unit": "GFLOP/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()
