@@ -125,8 +125,13 @@ lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* ctx, void* out_host, const void*
 unsigned long long lqcd_launch_count(void);
 
 /* Launch-geometry knobs for tuning runs; 0 restores the default.  Returns LQCD_EINVAL if the
- * value is not supported.  block_threads in {64,128,256}. */
+ * value is not supported.  block_threads in {64,128}. */
 lqcd_status lqcd_set_block_threads(lqcd_ctx* ctx, int block_threads);
+
+/* Link staging depth of the dslash kernel: 0 = links are loaded straight into registers; 4 or 8 =
+ * every thread streams its links into shared memory with cp.async that many hops ahead of use.
+ * -1 restores the default.  A performance knob only: results do not depend on it. */
+lqcd_status lqcd_set_link_stage_depth(lqcd_ctx* ctx, int depth);
 
 const char* lqcd_status_string(lqcd_status s);
 const char* lqcd_last_cuda_error(void); /* text of the last CUDA error seen by this thread's calls */

@@ -13,6 +13,9 @@
 
 namespace lqcd {
 
+__device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
+
 // unit coefficients: +1, -1, +i, -i
 enum Coef { C_P1 = 0, C_M1 = 1, C_PI = 2, C_MI = 3 };
 __host__ __device__ constexpr int coef_neg(int c) { return c ^ 1; }
@@ -27,6 +30,15 @@ __device__ __forceinline__ void cadd(R& dr, R& di, R sr, R si) {
     else { dr += si; di -= sr; }
 }
 
+// d += f * c * s for a unit coefficient c and a real factor f
+template <int C, typename R>
+__device__ __forceinline__ void cfma(R& dr, R& di, R f, R sr, R si) {
+    if (C == C_P1) { dr = fma_(f, sr, dr); di = fma_(f, si, di); }
+    else if (C == C_M1) { dr = fma_(-f, sr, dr); di = fma_(-f, si, di); }
+    else if (C == C_PI) { dr = fma_(-f, si, dr); di = fma_(f, sr, di); }
+    else { dr = fma_(f, si, dr); di = fma_(-f, sr, di); }
+}
+
 // Projection table: h0 = psi0 + S*ca*psi_ja, h1 = psi1 + S*cb*psi_jb; reconstruction
 // r2 = S*c2*chi_k2, r3 = S*c3*chi_k3, with S = +1 for (1 - gamma_mu) (forward hop) and
 // S = -1 for (1 + gamma_mu) (backward hop).  Derived from the gamma matrices above.
@@ -38,21 +50,12 @@ template <> struct Proj<3> { static constexpr int ja = 2, ca = C_P1, jb = 3, cb 
 
 template <typename R> struct BcPhases { R re[4], im[4]; };
 
-// One of the eight hops: gather neighbour spinor, project (K3), boundary phase (K3b),
-// colour multiply (K4), reconstruct + accumulate (K5).
-template <typename R, int RECON, bool CBC, int MU, bool FWD>
-__device__ __forceinline__ void hop(R acc[24], const R* __restrict__ gauge, const R* __restrict__ in,
-                                    const Geom& g, int cb, const Site& s, int p, const BcPhases<R>& bc) {
+// The arithmetic of one of the eight hops on a gathered neighbour spinor v and link u:
+// project (K3), boundary phase (K3b), colour multiply (K4), reconstruct + accumulate (K5).
+template <typename R, bool CBC, int MU, bool FWD>
+__device__ __forceinline__ void hop_math(R acc[24], const R v[24], const R u[18], bool cross, const BcPhases<R>& bc) {
     constexpr int S = FWD ? +1 : -1;
     using P = Proj<MU>;
-    bool cross;
-    const int nb = neighbour<MU, FWD>(g, cb, s, cross);
-
-    R v[24];
-    load_spinor<R>(in, g.Vh, nb, v);
-    R u[18];
-    // forward link U_mu(x) lives at x (parity p); backward link U_mu(x-mu^) at the neighbour (parity 1-p)
-    load_link<R, RECON>(gauge, g.Vh, FWD ? p : 1 - p, MU, FWD ? cb : nb, u);
 
     // K3: half spinor h[spin 2][colour 3][reim]
     R h[12];
@@ -66,7 +69,9 @@ __device__ __forceinline__ void hop(R acc[24], const R* __restrict__ gauge, cons
         h[6 + 2 * c] = r1; h[6 + 2 * c + 1] = i1;
     }
 
-    // K3b: psi(x + L mu^) = bc psi(x): forward crossing multiplies by bc_mu, backward by conj(bc_mu)
+    // K3b: psi(x + L mu^) = bc psi(x): forward crossing multiplies by bc_mu, backward by conj(bc_mu).
+    // Real (+-1) phases cost nothing: the sign f rides on the accumulation FMAs of K5.
+    R f = R(1);
     if (CBC) {
         if (cross) {
             const R br = bc.re[MU], bi = FWD ? bc.im[MU] : -bc.im[MU];
@@ -78,44 +83,79 @@ __device__ __forceinline__ void hop(R acc[24], const R* __restrict__ gauge, cons
             }
         }
     } else {
-        const R f = cross ? bc.re[MU] : R(1);  // +-1
-#pragma unroll
-        for (int k = 0; k < 12; ++k) h[k] *= f;
+        f = cross ? bc.re[MU] : R(1);
     }
 
-    // K4: chi = U h (forward) or U^+ h (backward), both spin components
+    // K4: chi = U h (forward) or U^+ h (backward), both spin components; explicit FMA chains
     R chi[12];
 #pragma unroll
     for (int sp = 0; sp < 2; ++sp)
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            R cr = 0, ci = 0;
+            R cr, ci;
 #pragma unroll
             for (int b = 0; b < 3; ++b) {
                 const R hr = h[6 * sp + 2 * b], hi = h[6 * sp + 2 * b + 1];
-                if (FWD) {
-                    const R ur = u[6 * a + 2 * b], ui = u[6 * a + 2 * b + 1];
-                    cr += ur * hr - ui * hi;
-                    ci += ur * hi + ui * hr;
-                } else {  // conj(U[b][a])
-                    const R ur = u[6 * b + 2 * a], ui = u[6 * b + 2 * a + 1];
-                    cr += ur * hr + ui * hi;
-                    ci += ur * hi - ui * hr;
+                // forward: U[a][b];  backward: conj(U[b][a])
+                const R ur = FWD ? u[6 * a + 2 * b] : u[6 * b + 2 * a];
+                const R ui = FWD ? u[6 * a + 2 * b + 1] : -u[6 * b + 2 * a + 1];
+                if (b == 0) {
+                    cr = ur * hr;
+                    ci = ur * hi;
+                } else {
+                    cr = fma_(ur, hr, cr);
+                    ci = fma_(ur, hi, ci);
                 }
+                cr = fma_(-ui, hi, cr);
+                ci = fma_(ui, hr, ci);
             }
             chi[6 * sp + 2 * a] = cr;
             chi[6 * sp + 2 * a + 1] = ci;
         }
 
-    // K5: out0 += chi0, out1 += chi1, out2 += S c2 chi_k2, out3 += S c3 chi_k3
+    // K5: out0 += f chi0, out1 += f chi1, out2 += f S c2 chi_k2, out3 += f S c3 chi_k3
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        acc[2 * c] += chi[2 * c];
-        acc[2 * c + 1] += chi[2 * c + 1];
-        acc[6 + 2 * c] += chi[6 + 2 * c];
-        acc[6 + 2 * c + 1] += chi[6 + 2 * c + 1];
-        cadd<coef_sgn<S>(P::c2)>(acc[12 + 2 * c], acc[12 + 2 * c + 1], chi[6 * P::k2 + 2 * c], chi[6 * P::k2 + 2 * c + 1]);
-        cadd<coef_sgn<S>(P::c3)>(acc[18 + 2 * c], acc[18 + 2 * c + 1], chi[6 * P::k3 + 2 * c], chi[6 * P::k3 + 2 * c + 1]);
+        acc[2 * c] = fma_(f, chi[2 * c], acc[2 * c]);
+        acc[2 * c + 1] = fma_(f, chi[2 * c + 1], acc[2 * c + 1]);
+        acc[6 + 2 * c] = fma_(f, chi[6 + 2 * c], acc[6 + 2 * c]);
+        acc[6 + 2 * c + 1] = fma_(f, chi[6 + 2 * c + 1], acc[6 + 2 * c + 1]);
+        cfma<coef_sgn<S>(P::c2)>(acc[12 + 2 * c], acc[12 + 2 * c + 1], f, chi[6 * P::k2 + 2 * c], chi[6 * P::k2 + 2 * c + 1]);
+        cfma<coef_sgn<S>(P::c3)>(acc[18 + 2 * c], acc[18 + 2 * c + 1], f, chi[6 * P::k3 + 2 * c], chi[6 * P::k3 + 2 * c + 1]);
+    }
+}
+
+// Hop K = 2 mu + (backward ? 1 : 0).  Forward link U_mu(x) lives at x (parity p); backward link
+// U_mu(x - mu^) at the neighbour (parity 1 - p).
+template <typename R, int RECON, int K>
+__device__ __forceinline__ const typename LinkWord<R, RECON>::type* hop_link_ptr(const R* __restrict__ gauge, int Vh, int p,
+                                                                                 int cb, const int nb[8]) {
+    constexpr int MU = K / 2;
+    constexpr bool FWD = (K & 1) == 0;
+    return link_ptr<R, RECON>(gauge, Vh, FWD ? p : 1 - p, MU, FWD ? cb : nb[K]);
+}
+
+template <typename R, int RECON, bool CBC, int BLOCK, int DEPTH, int K>
+__device__ __forceinline__ void hop_step(R acc[24], const R* __restrict__ gauge, const R* __restrict__ in, int Vh, int p,
+                                         int cb, const int nb[8], unsigned crossmask, const BcPhases<R>& bc,
+                                         LinkStage<R, RECON, BLOCK, (DEPTH > 0 ? DEPTH : 1)>& stage) {
+    constexpr int MU = K / 2;
+    constexpr bool FWD = (K & 1) == 0;
+    R v[24];
+    load_spinor<R>(in, Vh, nb[K], v);  // issued before the wait below: both latencies overlap
+    R u[18];
+    if constexpr (DEPTH == 0) {
+        load_link<R, RECON>(gauge, Vh, FWD ? p : 1 - p, MU, FWD ? cb : nb[K], u);
+    } else {
+        // groups committed so far: min(8, K + DEPTH); hop K's must be complete
+        constexpr int COMMITTED = (K + DEPTH < 8) ? K + DEPTH : 8;
+        cp_async_wait<COMMITTED - K - 1>();
+        stage.read(K, u);
+    }
+    hop_math<R, CBC, MU, FWD>(acc, v, u, (crossmask >> K) & 1u, bc);
+    if constexpr (DEPTH > 0 && K + DEPTH < 8) {
+        // slot K % DEPTH is free again (its words were consumed by the arithmetic above): refill it
+        stage.issue(K + DEPTH, hop_link_ptr<R, RECON, K + DEPTH>(gauge, Vh, p, cb, nb), Vh);
     }
 }
 
@@ -123,12 +163,13 @@ __device__ __forceinline__ void hop(R acc[24], const R* __restrict__ gauge, cons
 // out_p(x) = xin(x) + a (H in)(x)    (XPAY = true; a = -kappa or -kappa^2, step K6)
 // grid.y = 1: one parity `parity0`; grid.y = 2: both, parity = blockIdx.y, and in/out/xin are
 // full fields [even|odd] (in is read at the opposite half).
-template <typename R, int RECON, bool XPAY, bool CBC, int BLOCK>
+// DEPTH = 0: links loaded straight into registers; DEPTH = 4, 8: cp.async link staging DEPTH hops ahead
+// (dynamic shared memory = LinkStage::BYTES).
+template <typename R, int RECON, bool XPAY, bool CBC, int BLOCK, int DEPTH>
 __global__ void __launch_bounds__(BLOCK)
 dslash_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __restrict__ in,
               const R* __restrict__ xin, R a, Geom g, int parity0, BcPhases<R> bc) {
-    const int cb = blockIdx.x * BLOCK + threadIdx.x;
-    if (cb >= g.Vh) return;
+    extern __shared__ __align__(16) unsigned char smem[];
     int p = parity0;
     if (gridDim.y == 2) {
         p = blockIdx.y;
@@ -137,26 +178,57 @@ dslash_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __restr
         out += (size_t)p * half;
         if (XPAY) xin += (size_t)p * half;
     }
+    const int cb = blockIdx.x * BLOCK + threadIdx.x;
+    if (cb >= g.Vh) return;
     const Site s = decode_site(g, cb, p);
+
+    // K1: all eight neighbours and boundary-crossing flags up front
+    int nb[8];
+    unsigned crossmask = 0;
+    {
+        bool c;
+        nb[0] = neighbour<0, true>(g, cb, s, c);  crossmask |= (unsigned)c << 0;
+        nb[1] = neighbour<0, false>(g, cb, s, c); crossmask |= (unsigned)c << 1;
+        nb[2] = neighbour<1, true>(g, cb, s, c);  crossmask |= (unsigned)c << 2;
+        nb[3] = neighbour<1, false>(g, cb, s, c); crossmask |= (unsigned)c << 3;
+        nb[4] = neighbour<2, true>(g, cb, s, c);  crossmask |= (unsigned)c << 4;
+        nb[5] = neighbour<2, false>(g, cb, s, c); crossmask |= (unsigned)c << 5;
+        nb[6] = neighbour<3, true>(g, cb, s, c);  crossmask |= (unsigned)c << 6;
+        nb[7] = neighbour<3, false>(g, cb, s, c); crossmask |= (unsigned)c << 7;
+    }
+
+    LinkStage<R, RECON, BLOCK, (DEPTH > 0 ? DEPTH : 1)> stage(smem);
+    if constexpr (DEPTH > 0) {
+        stage.issue(0, hop_link_ptr<R, RECON, 0>(gauge, g.Vh, p, cb, nb), g.Vh);
+        stage.issue(1, hop_link_ptr<R, RECON, 1>(gauge, g.Vh, p, cb, nb), g.Vh);
+        stage.issue(2, hop_link_ptr<R, RECON, 2>(gauge, g.Vh, p, cb, nb), g.Vh);
+        stage.issue(3, hop_link_ptr<R, RECON, 3>(gauge, g.Vh, p, cb, nb), g.Vh);
+        if constexpr (DEPTH > 4) {
+            stage.issue(4, hop_link_ptr<R, RECON, 4>(gauge, g.Vh, p, cb, nb), g.Vh);
+            stage.issue(5, hop_link_ptr<R, RECON, 5>(gauge, g.Vh, p, cb, nb), g.Vh);
+            stage.issue(6, hop_link_ptr<R, RECON, 6>(gauge, g.Vh, p, cb, nb), g.Vh);
+            stage.issue(7, hop_link_ptr<R, RECON, 7>(gauge, g.Vh, p, cb, nb), g.Vh);
+        }
+    }
 
     R acc[24];
 #pragma unroll
     for (int k = 0; k < 24; ++k) acc[k] = 0;
 
-    hop<R, RECON, CBC, 0, true>(acc, gauge, in, g, cb, s, p, bc);
-    hop<R, RECON, CBC, 0, false>(acc, gauge, in, g, cb, s, p, bc);
-    hop<R, RECON, CBC, 1, true>(acc, gauge, in, g, cb, s, p, bc);
-    hop<R, RECON, CBC, 1, false>(acc, gauge, in, g, cb, s, p, bc);
-    hop<R, RECON, CBC, 2, true>(acc, gauge, in, g, cb, s, p, bc);
-    hop<R, RECON, CBC, 2, false>(acc, gauge, in, g, cb, s, p, bc);
-    hop<R, RECON, CBC, 3, true>(acc, gauge, in, g, cb, s, p, bc);
-    hop<R, RECON, CBC, 3, false>(acc, gauge, in, g, cb, s, p, bc);
+    hop_step<R, RECON, CBC, BLOCK, DEPTH, 0>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
+    hop_step<R, RECON, CBC, BLOCK, DEPTH, 1>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
+    hop_step<R, RECON, CBC, BLOCK, DEPTH, 2>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
+    hop_step<R, RECON, CBC, BLOCK, DEPTH, 3>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
+    hop_step<R, RECON, CBC, BLOCK, DEPTH, 4>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
+    hop_step<R, RECON, CBC, BLOCK, DEPTH, 5>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
+    hop_step<R, RECON, CBC, BLOCK, DEPTH, 6>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
+    hop_step<R, RECON, CBC, BLOCK, DEPTH, 7>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
 
     if (XPAY) {
         R x[24];
         load_spinor<R>(xin, g.Vh, cb, x);
 #pragma unroll
-        for (int k = 0; k < 24; ++k) acc[k] = x[k] + a * acc[k];
+        for (int k = 0; k < 24; ++k) acc[k] = fma_(a, acc[k], x[k]);
     }
     store_spinor<R>(out, g.Vh, cb, acc);
 }

@@ -10,6 +10,9 @@
 
 namespace lqcd {
 
+__device__ __forceinline__ float fmar(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fmar(double a, double b, double c) { return fma(a, b, c); }
+
 template <typename R> struct Word;            // 128-bit word of R
 template <> struct Word<float>  { using type = float4;  static constexpr int W = 4; };
 template <> struct Word<double> { using type = double2; static constexpr int W = 2; };
@@ -60,32 +63,90 @@ __device__ __forceinline__ float4  ld_stream(const float4* p)  { return __ldcs(p
 __device__ __forceinline__ float2  ld_stream(const float2* p)  { return __ldcs(p); }
 __device__ __forceinline__ double2 ld_stream(const double2* p) { return __ldcs(p); }
 
-// u[18]: row-major 3x3 complex, u[6 row + 2 col + reim].  RECON == 12 rebuilds row 2 as
-// conj(row0 x row1) (K2; valid for det U = +1; "RECONSTRUCT TWELVE").
+// K2: rebuild row 2 of u[18] (row-major 3x3 complex, u[6 row + 2 col + reim]) as conj(row0 x row1);
+// valid for det U = +1 ("RECONSTRUCT TWELVE").
+template <typename R>
+__device__ __forceinline__ void recon_row2(R u[18]) {
+    // row2[c] = conj(r0[a] r1[b] - r0[b] r1[a]),  (a,b) = (c+1, c+2) mod 3
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        const R ar = u[2 * a], ai = u[2 * a + 1], br = u[2 * b], bi = u[2 * b + 1];
+        const R cr = u[6 + 2 * b], ci = u[6 + 2 * b + 1], dr = u[6 + 2 * a], di = u[6 + 2 * a + 1];
+        const R re = fmar(-br, dr, fmar(bi, di, fmar(-ai, ci, ar * cr)));
+        const R im = fmar(-br, di, fmar(-bi, dr, fmar(ai, cr, ar * ci)));
+        u[12 + 2 * c] = re;
+        u[12 + 2 * c + 1] = -im;
+    }
+}
+
+// Address of word 0 of link (par, mu, cb); word w is Vh words further on.
+template <typename R, int RECON>
+__device__ __forceinline__ const typename LinkWord<R, RECON>::type* link_ptr(const R* __restrict__ gauge, int Vh,
+                                                                             int par, int mu, int cb) {
+    constexpr int NW = RECON / LinkWord<R, RECON>::LW;
+    return reinterpret_cast<const typename LinkWord<R, RECON>::type*>(gauge) + (size_t)((par * 4 + mu) * NW) * Vh + cb;
+}
+
+// L1: direct (register) link load + K2.
 template <typename R, int RECON>
 __device__ __forceinline__ void load_link(const R* __restrict__ gauge, int Vh, int par, int mu, int cb, R u[18]) {
     using LWd = typename LinkWord<R, RECON>::type;
     constexpr int LW = LinkWord<R, RECON>::LW, NW = RECON / LW;
-    const LWd* p = reinterpret_cast<const LWd*>(gauge) + (size_t)((par * 4 + mu) * NW) * Vh + cb;
+    const LWd* p = link_ptr<R, RECON>(gauge, Vh, par, mu, cb);
 #pragma unroll
     for (int w = 0; w < NW; ++w) {
         LWd x = ld_stream(p + (size_t)w * Vh);
         unpack(x, u + w * LW);
     }
-    if constexpr (RECON == 12) {
-        // row2[c] = conj(r0[a] r1[b] - r0[b] r1[a]),  (a,b) = (c+1, c+2) mod 3
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const int a = (c + 1) % 3, b = (c + 2) % 3;
-            const R ar = u[2 * a], ai = u[2 * a + 1], br = u[2 * b], bi = u[2 * b + 1];
-            const R cr = u[6 + 2 * b], ci = u[6 + 2 * b + 1], dr = u[6 + 2 * a], di = u[6 + 2 * a + 1];
-            // r0[a]*r1[b] - r0[b]*r1[a]
-            const R re = ar * cr - ai * ci - (br * dr - bi * di);
-            const R im = ar * ci + ai * cr - (br * di + bi * dr);
-            u[12 + 2 * c] = re;
-            u[12 + 2 * c + 1] = -im;
-        }
-    }
+    if constexpr (RECON == 12) recon_row2<R>(u);
 }
+
+// L1, staged: each thread streams its own links into shared memory with cp.async (LDGSTS) DEPTH hops
+// ahead of their use, so the DRAM-bound 2/3 of the traffic is in flight without holding registers.
+// A thread only ever reads back the words it copied itself, so no block-level barrier is needed:
+// cp.async.wait_group orders the copy before the read.  Slot layout [slot][word][thread], 16-byte
+// (8-byte for fp32 18-real) words: conflict-free for a warp.
+__device__ __forceinline__ void cp_async_word(float4* dst, const float4* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_word(double2* dst, const double2* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_word(float2* dst, const float2* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+template <typename R, int RECON, int BLOCK, int DEPTH>
+struct LinkStage {
+    using LWd = typename LinkWord<R, RECON>::type;
+    static constexpr int LW = LinkWord<R, RECON>::LW, NW = RECON / LW;
+    static constexpr size_t BYTES = (size_t)DEPTH * NW * BLOCK * sizeof(LWd);
+    LWd* mine;  // this thread's word 0 of slot 0
+
+    __device__ __forceinline__ explicit LinkStage(void* smem) : mine(static_cast<LWd*>(smem) + threadIdx.x) {}
+
+    // start the copy of one link into the slot of hop k, as one commit group
+    __device__ __forceinline__ void issue(int k, const LWd* src, int Vh) {
+        LWd* d = mine + (k % DEPTH) * NW * BLOCK;
+#pragma unroll
+        for (int w = 0; w < NW; ++w) cp_async_word(d + w * BLOCK, src + (size_t)w * Vh);
+        cp_async_commit();
+    }
+
+    // read hop k's link back (after cp_async_wait) and rebuild row 2
+    __device__ __forceinline__ void read(int k, R u[18]) const {
+        const LWd* d = mine + (k % DEPTH) * NW * BLOCK;
+#pragma unroll
+        for (int w = 0; w < NW; ++w) {
+            LWd x = d[w * BLOCK];
+            unpack(x, u + w * LW);
+        }
+        if constexpr (RECON == 12) recon_row2<R>(u);
+    }
+};
 
 }  // namespace lqcd

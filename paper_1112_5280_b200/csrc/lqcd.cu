@@ -18,7 +18,8 @@ struct lqcd_ctx {
     lqcd_params p;
     Geom g;
     bool complex_bc;
-    int block;  // threads per block of the dslash kernel
+    int block;    // threads per block of the dslash kernel
+    int depth;    // cp.async link staging depth in hops: 0 (register loads), 4 or 8
 };
 
 namespace {
@@ -58,13 +59,36 @@ BcPhases<R> make_bc(const lqcd_ctx* c) {
     return b;
 }
 
+template <typename R, int RECON, bool XPAY, bool CBC, int BLOCK, int DEPTH>
+lqcd_status launch_depth(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                         double a, int parity, cudaStream_t st) {
+    auto kern = dslash_kernel<R, RECON, XPAY, CBC, BLOCK, DEPTH>;
+    constexpr size_t smem = DEPTH > 0 ? LinkStage<R, RECON, BLOCK, (DEPTH > 0 ? DEPTH : 1)>::BYTES : 0;
+    if (smem > 48 * 1024) {
+        static thread_local int configured_device = -1;  // opt in to > 48 KB dynamic shared memory once per device
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (configured_device != dev) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return cuda_fail(e);
+            configured_device = dev;
+        }
+    }
+    const dim3 grid((c->g.Vh + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
+    kern<<<grid, BLOCK, smem, st>>>((R*)out, (const R*)gauge, (const R*)in, (const R*)xin, (R)a, c->g,
+                                    parity < 0 ? 0 : parity, make_bc<R>(c));
+    return after_launch();
+}
+
 template <typename R, int RECON, bool XPAY, bool CBC, int BLOCK>
 lqcd_status launch_block(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
                          double a, int parity, cudaStream_t st) {
-    const dim3 grid((c->g.Vh + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
-    dslash_kernel<R, RECON, XPAY, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
-        (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, (R)a, c->g, parity < 0 ? 0 : parity, make_bc<R>(c));
-    return after_launch();
+    switch (c->depth) {
+        case 0: return launch_depth<R, RECON, XPAY, CBC, BLOCK, 0>(c, out, gauge, in, xin, a, parity, st);
+        case 4: return launch_depth<R, RECON, XPAY, CBC, BLOCK, 4>(c, out, gauge, in, xin, a, parity, st);
+        case 8: return launch_depth<R, RECON, XPAY, CBC, BLOCK, 8>(c, out, gauge, in, xin, a, parity, st);
+    }
+    return LQCD_EUNSUPPORTED;
 }
 
 template <typename R, int RECON, bool XPAY, bool CBC>
@@ -73,7 +97,6 @@ lqcd_status launch_cbc(const lqcd_ctx* c, void* out, const void* gauge, const vo
     switch (c->block) {
         case 64: return launch_block<R, RECON, XPAY, CBC, 64>(c, out, gauge, in, xin, a, parity, st);
         case 128: return launch_block<R, RECON, XPAY, CBC, 128>(c, out, gauge, in, xin, a, parity, st);
-        case 256: return launch_block<R, RECON, XPAY, CBC, 256>(c, out, gauge, in, xin, a, parity, st);
     }
     return LQCD_EUNSUPPORTED;
 }
@@ -135,7 +158,8 @@ lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p) {
     g.Vh = g.Xh * g.Y * g.Z * g.T;
     g.sy = g.Xh; g.sz = g.Xh * g.Y; g.st = g.Xh * g.Y * g.Z;
     c->complex_bc = cbc;
-    c->block = 128;
+    c->block = 64;
+    c->depth = 0;
     *ctx = c;
     return LQCD_OK;
 }
@@ -157,9 +181,17 @@ size_t lqcd_host_workspace_bytes(const lqcd_ctx* c) {
 
 lqcd_status lqcd_set_block_threads(lqcd_ctx* c, int b) {
     if (!c) return LQCD_EINVAL;
-    if (b == 0) b = 128;
-    if (b != 64 && b != 128 && b != 256) return LQCD_EINVAL;
+    if (b == 0) b = 64;
+    if (b != 64 && b != 128) return LQCD_EINVAL;
     c->block = b;
+    return LQCD_OK;
+}
+
+lqcd_status lqcd_set_link_stage_depth(lqcd_ctx* c, int depth) {
+    if (!c) return LQCD_EINVAL;
+    if (depth < 0) depth = 0;
+    if (depth != 0 && depth != 4 && depth != 8) return LQCD_EINVAL;
+    c->depth = depth;
     return LQCD_OK;
 }
 

@@ -46,9 +46,12 @@ def test_create_validation_and_sizes():
         with pytest.raises(L.LqcdError) as e:
             L.Context(**kw)
         assert e.value.status == L.LQCD_EINVAL
-    c.set_block_threads(256)
+    c.set_block_threads(128)
     with pytest.raises(L.LqcdError):
         c.set_block_threads(100)
+    c.set_link_stage_depth(8)
+    with pytest.raises(L.LqcdError):
+        c.set_link_stage_depth(3)
 
 
 def test_null_pointers_rejected_without_gpu():
