@@ -51,7 +51,6 @@ def parse_args():
     ap.add_argument("--precision", type=int, default=32, choices=[32, 64], help="precision of the primary line")
     ap.add_argument("--recon", type=int, default=12, choices=[12, 18])
     ap.add_argument("--block", type=int, default=0, help="dslash block size override (tuning)")
-    ap.add_argument("--depth", type=int, default=-1, help="cp.async link staging depth 0/4/8 (tuning; -1 = library default)")
     ap.add_argument("--chain", action="store_true", help="also time config 5: apply_M(eo=1) x100 chained at 48^3x96")
     ap.add_argument("--no-extras", action="store_true", help="skip the fp64 / chain / e2e / cpu legs (profiling runs)")
     return ap.parse_args()
@@ -135,7 +134,7 @@ class ClockSampler:
 class Workload:
     """Seeded inputs of one config on the device in native layout, plus pinned host copies."""
 
-    def __init__(self, cfg_id, precision, recon, dev, block=0, nbuf=NBUF, keep_host=True, in_parity=None, depth=-1):
+    def __init__(self, cfg_id, precision, recon, dev, block=0, nbuf=NBUF, keep_host=True, in_parity=None):
         import numpy as np
         import torch
         import lattice_inputs as li
@@ -148,8 +147,6 @@ class Workload:
         self.ctx = L.Context(self.dims, precision, recon, self.bc)
         if block:
             self.ctx.set_block_threads(block)
-        if depth >= 0:
-            self.ctx.set_link_stage_depth(depth)
         self.Vh = self.ctx.Vh
         U = li.links_for_config(cfg_id, dtype=cd)
         self.U_host = torch.from_numpy(U).pin_memory() if keep_host else None
@@ -348,7 +345,7 @@ def run_b200(args):
     L._lib()
     peak, peak_src = measured_peaks()
 
-    w = Workload(args.config, args.precision, args.recon, dev, args.block, depth=args.depth)
+    w = Workload(args.config, args.precision, args.recon, dev, args.block)
     sampler = ClockSampler(local) if rank == 0 else None
     t0 = time.time()
     main = kernel_leg(torch, dist, w, args.steps, args.warmup, world)
@@ -394,7 +391,7 @@ def run_b200(args):
     torch.cuda.empty_cache()
     if not args.no_extras:
         other = 64 if args.precision == 32 else 32
-        w2 = Workload(args.config, other, args.recon, dev, args.block, keep_host=False, depth=args.depth)
+        w2 = Workload(args.config, other, args.recon, dev, args.block, keep_host=False)
         r2 = kernel_leg(torch, dist, w2, max(1, args.steps // 2), args.warmup, world)
         line[f"fp{other}"] = {"gflops": r2["gflops"], "achieved_gbs": r2["gbs"], "frac": r2["gbs"] / peak,
                               "frac_of_nominal_8TBs": r2["gbs"] / NOMINAL_HBM_GBS, "us_per_launch": r2["us_per_launch"],

@@ -32,13 +32,19 @@
  *     half spinor  [V/2][spin 4][colour 3]  -- the sites of one parity in increasing
  *                  lexicographic order lex = x + X(y + Y(z + Z t)), i.e. indexed by cb = lex >> 1
  *     links        [mu 4][T][Z][Y][X][row 3][col 3],  (U psi)_a = sum_b U[a][b] psi_b,  U_mu(x) at x
- *   native (what the hot path reads/writes; structure of arrays, site-fastest, checkerboarded)
+ *   native (what the hot path reads/writes; array of structures of arrays, checkerboarded, warp tiles)
+ *     Sites of one parity are numbered by cb and grouped in tiles of 32 consecutive cb;
+ *     ntiles = ceil(V/2 / 32), the last tile is padded (padding is never read or written).
  *     real component r = 6 spin + 2 colour + reim (spinor, 24) or 6 row + 2 col + reim (link,
  *     first `recon` reals of 18).  W = 16 bytes / sizeof(element) reals per 128-bit word.
- *     half spinor  word q = r / W, lane = r % W  at  element index (q * V/2 + cb) * W + lane
- *     full spinor  [even half | odd half]
- *     links        [parity of base site 2][mu 4][word][V/2][lane]; words of 4 floats (recon 12,
- *                  3 words), 2 floats (precision 32 recon 18, 9 words of 8 bytes) or 2 doubles.
+ *     half spinor  word q = r / W, lane = r % W  at element ((cb/32 * 24/W + q) * 32 + cb%32) * W + lane
+ *     full spinor  [even half | odd half], each of lqcd_spinor_bytes(ctx, 1) bytes
+ *     links        gathered by output site: [parity p of x][tile][hop k 8][word][32][lane], hop k = 2 mu holds
+ *                  U_mu(x), k = 2 mu + 1 holds U_mu(x - mu^) (stored as is; the kernel takes the adjoint).
+ *                  Words of 4 floats (recon 12, 3 words), 2 floats (precision 32 recon 18, 9 words of
+ *                  8 bytes) or 2 doubles.  Every link is stored twice (capacity for contiguity: all
+ *                  8 links of a warp's 32 sites form one contiguous block); one application of
+ *                  lqcd_dslash_eo still reads 8 links per output site exactly once.
  */
 #ifndef LQCD_H
 #define LQCD_H
@@ -79,7 +85,7 @@ lqcd_status lqcd_destroy(lqcd_ctx* ctx); /* NULL is a no-op */
 
 /* Sizes in bytes of native buffers for this ctx (0 if ctx is NULL). */
 size_t lqcd_spinor_bytes(const lqcd_ctx* ctx, int half); /* half != 0: one parity; 0: full [even|odd] */
-size_t lqcd_gauge_bytes(const lqcd_ctx* ctx);            /* native links, 2*4*recon*V/2 elements */
+size_t lqcd_gauge_bytes(const lqcd_ctx* ctx);            /* native links, 2*8*recon*32*ntiles elements */
 size_t lqcd_workspace_bytes(const lqcd_ctx* ctx);        /* lqcd_apply_M(eo=1): one native half spinor */
 size_t lqcd_host_workspace_bytes(const lqcd_ctx* ctx);   /* device scratch of lqcd_dslash_eo_host */
 
@@ -127,11 +133,6 @@ unsigned long long lqcd_launch_count(void);
 /* Launch-geometry knobs for tuning runs; 0 restores the default.  Returns LQCD_EINVAL if the
  * value is not supported.  block_threads in {64,128}. */
 lqcd_status lqcd_set_block_threads(lqcd_ctx* ctx, int block_threads);
-
-/* Link staging depth of the dslash kernel: 0 = links are loaded straight into registers; 4 or 8 =
- * every thread streams its links into shared memory with cp.async that many hops ahead of use.
- * -1 restores the default.  A performance knob only: results do not depend on it. */
-lqcd_status lqcd_set_link_stage_depth(lqcd_ctx* ctx, int depth);
 
 const char* lqcd_status_string(lqcd_status s);
 const char* lqcd_last_cuda_error(void); /* text of the last CUDA error seen by this thread's calls */

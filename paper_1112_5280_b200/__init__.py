@@ -19,7 +19,7 @@ EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
     "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_dslash_eo_host", "lqcd_launch_count",
-    "lqcd_set_block_threads", "lqcd_set_link_stage_depth", "lqcd_status_string", "lqcd_last_cuda_error",
+    "lqcd_set_block_threads", "lqcd_status_string", "lqcd_last_cuda_error",
 ]
 
 
@@ -66,7 +66,6 @@ def _lib():
         lib.lqcd_launch_count.argtypes = []
         lib.lqcd_launch_count.restype = ctypes.c_ulonglong
         lib.lqcd_set_block_threads.argtypes = [vp, ci]
-        lib.lqcd_set_link_stage_depth.argtypes = [vp, ci]
         lib.lqcd_status_string.argtypes = [ci]
         lib.lqcd_status_string.restype = ctypes.c_char_p
         lib.lqcd_last_cuda_error.argtypes = []
@@ -126,9 +125,6 @@ class Context:
 
     def set_block_threads(self, n):
         _chk(_lib().lqcd_set_block_threads(self._h, int(n)), "lqcd_set_block_threads")
-
-    def set_link_stage_depth(self, depth):
-        _chk(_lib().lqcd_set_link_stage_depth(self._h, int(depth)), "lqcd_set_link_stage_depth")
 
     # layout conversion
     def pack_gauge(self, native, canonical, stream=None):

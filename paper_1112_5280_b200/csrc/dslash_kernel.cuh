@@ -125,55 +125,54 @@ __device__ __forceinline__ void hop_math(R acc[24], const R v[24], const R u[18]
     }
 }
 
-// Hop K = 2 mu + (backward ? 1 : 0).  Forward link U_mu(x) lives at x (parity p); backward link
-// U_mu(x - mu^) at the neighbour (parity 1 - p).
-template <typename R, int RECON, int K>
-__device__ __forceinline__ const typename LinkWord<R, RECON>::type* hop_link_ptr(const R* __restrict__ gauge, int Vh, int p,
-                                                                                 int cb, const int nb[8]) {
+// Hop K = 2 mu + (backward ? 1 : 0): gather the neighbour spinor and the link stored for this hop
+// (U_mu(x) or U_mu(x - mu^), fields.cuh), then the arithmetic.
+template <typename R, int RECON, bool CBC, int K>
+__device__ __forceinline__ void hop_step(R acc[24], const typename LinkWord<R, RECON>::type* __restrict__ site_links,
+                                         const R* __restrict__ in, const int nb[8], unsigned crossmask,
+                                         const BcPhases<R>& bc) {
     constexpr int MU = K / 2;
     constexpr bool FWD = (K & 1) == 0;
-    return link_ptr<R, RECON>(gauge, Vh, FWD ? p : 1 - p, MU, FWD ? cb : nb[K]);
+    R v[24], u[18];
+    load_spinor<R>(in, nb[K], v);
+    load_link<R, RECON>(site_links, K, u);
+    hop_math<R, CBC, MU, FWD>(acc, v, u, (crossmask >> K) & 1u, bc);
 }
 
-template <typename R, int RECON, bool CBC, int BLOCK, int DEPTH, int K>
-__device__ __forceinline__ void hop_step(R acc[24], const R* __restrict__ gauge, const R* __restrict__ in, int Vh, int p,
-                                         int cb, const int nb[8], unsigned crossmask, const BcPhases<R>& bc,
-                                         LinkStage<R, RECON, BLOCK, (DEPTH > 0 ? DEPTH : 1)>& stage) {
-    constexpr int MU = K / 2;
-    constexpr bool FWD = (K & 1) == 0;
-    R v[24];
-    load_spinor<R>(in, Vh, nb[K], v);  // issued before the wait below: both latencies overlap
-    R u[18];
-    if constexpr (DEPTH == 0) {
-        load_link<R, RECON>(gauge, Vh, FWD ? p : 1 - p, MU, FWD ? cb : nb[K], u);
-    } else {
-        // groups committed so far: min(8, K + DEPTH); hop K's must be complete
-        constexpr int COMMITTED = (K + DEPTH < 8) ? K + DEPTH : 8;
-        cp_async_wait<COMMITTED - K - 1>();
-        stage.read(K, u);
-    }
-    hop_math<R, CBC, MU, FWD>(acc, v, u, (crossmask >> K) & 1u, bc);
-    if constexpr (DEPTH > 0 && K + DEPTH < 8) {
-        // slot K % DEPTH is free again (its words were consumed by the arithmetic above): refill it
-        stage.issue(K + DEPTH, hop_link_ptr<R, RECON, K + DEPTH>(gauge, Vh, p, cb, nb), Vh);
-    }
-}
+// Resident 64-thread blocks per SM promised to ptxas (__launch_bounds__ min blocks).  The hint sets the
+// register budget (65536 / (64 value)), and ptxas spends whatever budget it is given on hoisting the
+// gathers ahead of their use, so it fixes the balance between loads in flight per thread and threads
+// per SM.  Values measured on B200 at 32^3x64 (profiles/r01_varsweep_minblocks.txt); overridable for sweeps.
+#ifndef LQCD_MINB_F32_R12
+#define LQCD_MINB_F32_R12 8
+#endif
+#ifndef LQCD_MINB_F32_R18
+#define LQCD_MINB_F32_R18 6
+#endif
+#ifndef LQCD_MINB_F64_R12
+#define LQCD_MINB_F64_R12 6
+#endif
+#ifndef LQCD_MINB_F64_R18
+#define LQCD_MINB_F64_R18 4
+#endif
+template <typename R, int RECON> struct MinBlocks;
+template <> struct MinBlocks<float, 12>  { static constexpr int value = LQCD_MINB_F32_R12; };
+template <> struct MinBlocks<float, 18>  { static constexpr int value = LQCD_MINB_F32_R18; };
+template <> struct MinBlocks<double, 12> { static constexpr int value = LQCD_MINB_F64_R12; };
+template <> struct MinBlocks<double, 18> { static constexpr int value = LQCD_MINB_F64_R18; };
 
 // out_p(x) = (H in)(x)              (XPAY = false)
 // out_p(x) = xin(x) + a (H in)(x)    (XPAY = true; a = -kappa or -kappa^2, step K6)
 // grid.y = 1: one parity `parity0`; grid.y = 2: both, parity = blockIdx.y, and in/out/xin are
-// full fields [even|odd] (in is read at the opposite half).
-// DEPTH = 0: links loaded straight into registers; DEPTH = 4, 8: cp.async link staging DEPTH hops ahead
-// (dynamic shared memory = LinkStage::BYTES).
-template <typename R, int RECON, bool XPAY, bool CBC, int BLOCK, int DEPTH>
-__global__ void __launch_bounds__(BLOCK)
+// full fields [even|odd] (in is read at the opposite half).  One thread per output site.
+template <typename R, int RECON, bool XPAY, bool CBC, int BLOCK>
+__global__ void __launch_bounds__(BLOCK, MinBlocks<R, RECON>::value * 64 / BLOCK)
 dslash_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __restrict__ in,
               const R* __restrict__ xin, R a, Geom g, int parity0, BcPhases<R> bc) {
-    extern __shared__ __align__(16) unsigned char smem[];
     int p = parity0;
     if (gridDim.y == 2) {
         p = blockIdx.y;
-        const size_t half = (size_t)24 * g.Vh;
+        const size_t half = (size_t)24 * TILE * g.ntiles;
         in += (size_t)(1 - p) * half;
         out += (size_t)p * half;
         if (XPAY) xin += (size_t)p * half;
@@ -182,7 +181,7 @@ dslash_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __restr
     if (cb >= g.Vh) return;
     const Site s = decode_site(g, cb, p);
 
-    // K1: all eight neighbours and boundary-crossing flags up front
+    // K1: all eight neighbours and boundary-crossing flags
     int nb[8];
     unsigned crossmask = 0;
     {
@@ -196,41 +195,29 @@ dslash_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __restr
         nb[6] = neighbour<3, true>(g, cb, s, c);  crossmask |= (unsigned)c << 6;
         nb[7] = neighbour<3, false>(g, cb, s, c); crossmask |= (unsigned)c << 7;
     }
-
-    LinkStage<R, RECON, BLOCK, (DEPTH > 0 ? DEPTH : 1)> stage(smem);
-    if constexpr (DEPTH > 0) {
-        stage.issue(0, hop_link_ptr<R, RECON, 0>(gauge, g.Vh, p, cb, nb), g.Vh);
-        stage.issue(1, hop_link_ptr<R, RECON, 1>(gauge, g.Vh, p, cb, nb), g.Vh);
-        stage.issue(2, hop_link_ptr<R, RECON, 2>(gauge, g.Vh, p, cb, nb), g.Vh);
-        stage.issue(3, hop_link_ptr<R, RECON, 3>(gauge, g.Vh, p, cb, nb), g.Vh);
-        if constexpr (DEPTH > 4) {
-            stage.issue(4, hop_link_ptr<R, RECON, 4>(gauge, g.Vh, p, cb, nb), g.Vh);
-            stage.issue(5, hop_link_ptr<R, RECON, 5>(gauge, g.Vh, p, cb, nb), g.Vh);
-            stage.issue(6, hop_link_ptr<R, RECON, 6>(gauge, g.Vh, p, cb, nb), g.Vh);
-            stage.issue(7, hop_link_ptr<R, RECON, 7>(gauge, g.Vh, p, cb, nb), g.Vh);
-        }
-    }
+    const auto* site_links =
+        reinterpret_cast<const typename LinkWord<R, RECON>::type*>(gauge) + link_word0<R, RECON>(g.ntiles, p, cb, 0);
 
     R acc[24];
 #pragma unroll
     for (int k = 0; k < 24; ++k) acc[k] = 0;
 
-    hop_step<R, RECON, CBC, BLOCK, DEPTH, 0>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
-    hop_step<R, RECON, CBC, BLOCK, DEPTH, 1>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
-    hop_step<R, RECON, CBC, BLOCK, DEPTH, 2>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
-    hop_step<R, RECON, CBC, BLOCK, DEPTH, 3>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
-    hop_step<R, RECON, CBC, BLOCK, DEPTH, 4>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
-    hop_step<R, RECON, CBC, BLOCK, DEPTH, 5>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
-    hop_step<R, RECON, CBC, BLOCK, DEPTH, 6>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
-    hop_step<R, RECON, CBC, BLOCK, DEPTH, 7>(acc, gauge, in, g.Vh, p, cb, nb, crossmask, bc, stage);
+    hop_step<R, RECON, CBC, 0>(acc, site_links, in, nb, crossmask, bc);
+    hop_step<R, RECON, CBC, 1>(acc, site_links, in, nb, crossmask, bc);
+    hop_step<R, RECON, CBC, 2>(acc, site_links, in, nb, crossmask, bc);
+    hop_step<R, RECON, CBC, 3>(acc, site_links, in, nb, crossmask, bc);
+    hop_step<R, RECON, CBC, 4>(acc, site_links, in, nb, crossmask, bc);
+    hop_step<R, RECON, CBC, 5>(acc, site_links, in, nb, crossmask, bc);
+    hop_step<R, RECON, CBC, 6>(acc, site_links, in, nb, crossmask, bc);
+    hop_step<R, RECON, CBC, 7>(acc, site_links, in, nb, crossmask, bc);
 
     if (XPAY) {
         R x[24];
-        load_spinor<R>(xin, g.Vh, cb, x);
+        load_spinor<R>(xin, cb, x);
 #pragma unroll
         for (int k = 0; k < 24; ++k) acc[k] = fma_(a, acc[k], x[k]);
     }
-    store_spinor<R>(out, g.Vh, cb, acc);
+    store_spinor<R>(out, cb, acc);
 }
 
 }  // namespace lqcd

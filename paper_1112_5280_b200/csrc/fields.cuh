@@ -1,14 +1,24 @@
 // fields.cuh -- native field layout (step L0) and 128-bit loads/stores (L1, L2, L6), K2 recon.
 //
-// Native layout (include/lqcd.h):
-//   spinor: real r = 6 spin + 2 colour + reim in [0,24); W = 16/sizeof(R) reals per word;
-//           word q = r / W of site cb at word index q * Vh + cb  (consecutive sites adjacent).
-//   links:  real r = 6 row + 2 col + reim over the first RECON reals; words of LW reals;
-//           array [parity][mu][word][Vh].
+// Native layout (include/lqcd.h): array of structures of arrays with
+// warp-sized tiles.  Sites of one parity are numbered by their checkerboard index cb and grouped in
+// tiles of TILE = 32 consecutive cb (one warp); ntiles = ceil(Vh / 32), the last tile is padded.
+//   spinor: real r = 6 spin + 2 colour + reim in [0,24); W = 16/sizeof(R) reals per 16-byte word,
+//           Q = 24 / W words; word q of site cb at word index ((cb / 32) * Q + q) * 32 + cb % 32.
+//           A warp reads word q of its 32 sites as one 512-byte run, and the Q words of a tile are
+//           adjacent: one contiguous 1.5 KB (fp32) / 3 KB (fp64) block per warp-level gather.
+//   links:  "gathered by output site": for the site cb of parity p, hop k = 2 mu + (backward ? 1 : 0)
+//           holds U_mu(x) (k even) or U_mu(x - mu^) (k odd), first RECON reals r = 6 row + 2 col + reim,
+//           in words of LW reals; word w at ((((p * ntiles + cb / 32) * 8 + k) * NW + w) * 32 + cb % 32.
+//           All 8 links of a warp's sites are one contiguous block read front to back (12 KB fp32
+//           recon-12); every link is stored twice (as the forward link of x and the backward link of
+//           x + mu^), which costs capacity, not traffic: one application reads each copy it needs once.
 #pragma once
 #include <cuda_runtime.h>
 
 namespace lqcd {
+
+constexpr int TILE = 32;
 
 __device__ __forceinline__ float fmar(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ double fmar(double a, double b, double c) { return fma(a, b, c); }
@@ -27,33 +37,44 @@ __device__ __forceinline__ void unpack(const double2& w, double* v) { v[0] = w.x
 __device__ __forceinline__ float4  pack4(const float* v)  { return make_float4(v[0], v[1], v[2], v[3]); }
 __device__ __forceinline__ double2 pack2(const double* v) { return make_double2(v[0], v[1]); }
 
+// word 0 of site cb in a native half spinor; word q is q * TILE words further on
+template <typename R>
+__host__ __device__ __forceinline__ size_t spinor_word0(int cb) {
+    constexpr int Q = 24 / Word<R>::W;
+    return (size_t)(cb / TILE) * (Q * TILE) + (cb % TILE);
+}
+
+// word 0 of hop k's link of site cb (parity p); word w is w * TILE words further on
+template <typename R, int RECON>
+__host__ __device__ __forceinline__ size_t link_word0(int ntiles, int p, int cb, int k) {
+    constexpr int NW = RECON / LinkWord<R, RECON>::LW;
+    return ((size_t)(p * ntiles + cb / TILE) * 8 + k) * (NW * TILE) + (cb % TILE);
+}
+
 // Spinor loads take the default cached path: each input spinor is gathered by 8 output
 // sites, and that reuse must come from L1/L2, not from DRAM.
 template <typename R>
-__device__ __forceinline__ void load_spinor(const R* __restrict__ base, int Vh, int cb, R v[24]) {
+__device__ __forceinline__ void load_spinor(const R* __restrict__ base, int cb, R v[24]) {
     using Wd = typename Word<R>::type;
     constexpr int W = Word<R>::W, Q = 24 / W;
-    const Wd* p = reinterpret_cast<const Wd*>(base) + cb;
+    const Wd* p = reinterpret_cast<const Wd*>(base) + spinor_word0<R>(cb);
 #pragma unroll
     for (int q = 0; q < Q; ++q) {
-        Wd w = __ldg(p + (size_t)q * Vh);
+        Wd w = __ldg(p + q * TILE);
         unpack(w, v + q * W);
     }
 }
 
-__device__ __forceinline__ void st_stream(float4* p, float4 v)  { __stcs(p, v); }
-__device__ __forceinline__ void st_stream(double2* p, double2 v) { __stcs(p, v); }
-
 template <typename R>
-__device__ __forceinline__ void store_spinor(R* __restrict__ base, int Vh, int cb, const R v[24]) {
+__device__ __forceinline__ void store_spinor(R* __restrict__ base, int cb, const R v[24]) {
     using Wd = typename Word<R>::type;
     constexpr int W = Word<R>::W, Q = 24 / W;
-    Wd* p = reinterpret_cast<Wd*>(base) + cb;
+    Wd* p = reinterpret_cast<Wd*>(base) + spinor_word0<R>(cb);
 #pragma unroll
     for (int q = 0; q < Q; ++q) {
         Wd w;
         if constexpr (W == 4) w = pack4(v + q * W); else w = pack2(v + q * W);
-        p[(size_t)q * Vh] = w;
+        p[q * TILE] = w;
     }
 }
 
@@ -80,73 +101,17 @@ __device__ __forceinline__ void recon_row2(R u[18]) {
     }
 }
 
-// Address of word 0 of link (par, mu, cb); word w is Vh words further on.
+// L1 + K2: link of hop k for the site whose hop-0 word-0 address is `site_links`.
 template <typename R, int RECON>
-__device__ __forceinline__ const typename LinkWord<R, RECON>::type* link_ptr(const R* __restrict__ gauge, int Vh,
-                                                                             int par, int mu, int cb) {
-    constexpr int NW = RECON / LinkWord<R, RECON>::LW;
-    return reinterpret_cast<const typename LinkWord<R, RECON>::type*>(gauge) + (size_t)((par * 4 + mu) * NW) * Vh + cb;
-}
-
-// L1: direct (register) link load + K2.
-template <typename R, int RECON>
-__device__ __forceinline__ void load_link(const R* __restrict__ gauge, int Vh, int par, int mu, int cb, R u[18]) {
+__device__ __forceinline__ void load_link(const typename LinkWord<R, RECON>::type* __restrict__ site_links, int k, R u[18]) {
     using LWd = typename LinkWord<R, RECON>::type;
     constexpr int LW = LinkWord<R, RECON>::LW, NW = RECON / LW;
-    const LWd* p = link_ptr<R, RECON>(gauge, Vh, par, mu, cb);
 #pragma unroll
     for (int w = 0; w < NW; ++w) {
-        LWd x = ld_stream(p + (size_t)w * Vh);
+        LWd x = ld_stream(site_links + (k * NW + w) * TILE);
         unpack(x, u + w * LW);
     }
     if constexpr (RECON == 12) recon_row2<R>(u);
 }
-
-// L1, staged: each thread streams its own links into shared memory with cp.async (LDGSTS) DEPTH hops
-// ahead of their use, so the DRAM-bound 2/3 of the traffic is in flight without holding registers.
-// A thread only ever reads back the words it copied itself, so no block-level barrier is needed:
-// cp.async.wait_group orders the copy before the read.  Slot layout [slot][word][thread], 16-byte
-// (8-byte for fp32 18-real) words: conflict-free for a warp.
-__device__ __forceinline__ void cp_async_word(float4* dst, const float4* src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_word(double2* dst, const double2* src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_word(float2* dst, const float2* src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-template <typename R, int RECON, int BLOCK, int DEPTH>
-struct LinkStage {
-    using LWd = typename LinkWord<R, RECON>::type;
-    static constexpr int LW = LinkWord<R, RECON>::LW, NW = RECON / LW;
-    static constexpr size_t BYTES = (size_t)DEPTH * NW * BLOCK * sizeof(LWd);
-    LWd* mine;  // this thread's word 0 of slot 0
-
-    __device__ __forceinline__ explicit LinkStage(void* smem) : mine(static_cast<LWd*>(smem) + threadIdx.x) {}
-
-    // start the copy of one link into the slot of hop k, as one commit group
-    __device__ __forceinline__ void issue(int k, const LWd* src, int Vh) {
-        LWd* d = mine + (k % DEPTH) * NW * BLOCK;
-#pragma unroll
-        for (int w = 0; w < NW; ++w) cp_async_word(d + w * BLOCK, src + (size_t)w * Vh);
-        cp_async_commit();
-    }
-
-    // read hop k's link back (after cp_async_wait) and rebuild row 2
-    __device__ __forceinline__ void read(int k, R u[18]) const {
-        const LWd* d = mine + (k % DEPTH) * NW * BLOCK;
-#pragma unroll
-        for (int w = 0; w < NW; ++w) {
-            LWd x = d[w * BLOCK];
-            unpack(x, u + w * LW);
-        }
-        if constexpr (RECON == 12) recon_row2<R>(u);
-    }
-};
 
 }  // namespace lqcd

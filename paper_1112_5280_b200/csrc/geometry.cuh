@@ -13,6 +13,7 @@ struct Geom {
     int X, Y, Z, T;  // extents
     int Xh;          // X / 2
     int Vh;          // X*Y*Z*T / 2 (sites per parity)
+    int ntiles;      // ceil(Vh / 32): 32-site tiles per parity in the native layout (fields.cuh)
     int sy, sz, st;  // cb strides of y, z, t: Xh, Xh*Y, Xh*Y*Z
 };
 

@@ -19,7 +19,6 @@ struct lqcd_ctx {
     Geom g;
     bool complex_bc;
     int block;    // threads per block of the dslash kernel
-    int depth;    // cp.async link staging depth in hops: 0 (register loads), 4 or 8
 };
 
 namespace {
@@ -46,7 +45,7 @@ inline bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
 }
 
 inline size_t elem(const lqcd_ctx* c) { return c->p.precision == 32 ? 4 : 8; }
-inline size_t half_bytes(const lqcd_ctx* c) { return (size_t)24 * c->g.Vh * elem(c); }
+inline size_t half_bytes(const lqcd_ctx* c) { return (size_t)24 * TILE * c->g.ntiles * elem(c); }  // padded to whole tiles
 inline size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
 
 template <typename R>
@@ -59,36 +58,13 @@ BcPhases<R> make_bc(const lqcd_ctx* c) {
     return b;
 }
 
-template <typename R, int RECON, bool XPAY, bool CBC, int BLOCK, int DEPTH>
-lqcd_status launch_depth(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                         double a, int parity, cudaStream_t st) {
-    auto kern = dslash_kernel<R, RECON, XPAY, CBC, BLOCK, DEPTH>;
-    constexpr size_t smem = DEPTH > 0 ? LinkStage<R, RECON, BLOCK, (DEPTH > 0 ? DEPTH : 1)>::BYTES : 0;
-    if (smem > 48 * 1024) {
-        static thread_local int configured_device = -1;  // opt in to > 48 KB dynamic shared memory once per device
-        int dev = 0;
-        cudaGetDevice(&dev);
-        if (configured_device != dev) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (e != cudaSuccess) return cuda_fail(e);
-            configured_device = dev;
-        }
-    }
-    const dim3 grid((c->g.Vh + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
-    kern<<<grid, BLOCK, smem, st>>>((R*)out, (const R*)gauge, (const R*)in, (const R*)xin, (R)a, c->g,
-                                    parity < 0 ? 0 : parity, make_bc<R>(c));
-    return after_launch();
-}
-
 template <typename R, int RECON, bool XPAY, bool CBC, int BLOCK>
 lqcd_status launch_block(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
                          double a, int parity, cudaStream_t st) {
-    switch (c->depth) {
-        case 0: return launch_depth<R, RECON, XPAY, CBC, BLOCK, 0>(c, out, gauge, in, xin, a, parity, st);
-        case 4: return launch_depth<R, RECON, XPAY, CBC, BLOCK, 4>(c, out, gauge, in, xin, a, parity, st);
-        case 8: return launch_depth<R, RECON, XPAY, CBC, BLOCK, 8>(c, out, gauge, in, xin, a, parity, st);
-    }
-    return LQCD_EUNSUPPORTED;
+    const dim3 grid((c->g.Vh + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
+    dslash_kernel<R, RECON, XPAY, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
+        (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, (R)a, c->g, parity < 0 ? 0 : parity, make_bc<R>(c));
+    return after_launch();
 }
 
 template <typename R, int RECON, bool XPAY, bool CBC>
@@ -147,8 +123,8 @@ lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p) {
         if (!(std::fabs(n2 - 1.0) <= 1e-12)) return LQCD_EINVAL;
         if (p->bc_im[mu] != 0.0) cbc = true;
     }
-    // word indices (12 words x Vh per half spinor in fp64, 2*4*9*Vh link words) are kept below 2^31
-    if (vol / 2 * 72 >= 2147483648.0) return LQCD_EUNSUPPORTED;
+    // checkerboard indices and in-tile word offsets are 32-bit; field offsets are size_t
+    if (vol / 2 >= 1073741824.0) return LQCD_EUNSUPPORTED;
     lqcd_ctx* c = new (std::nothrow) lqcd_ctx;
     if (!c) return LQCD_EINVAL;
     c->p = *p;
@@ -156,10 +132,10 @@ lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p) {
     g.X = p->dims[0]; g.Y = p->dims[1]; g.Z = p->dims[2]; g.T = p->dims[3];
     g.Xh = g.X / 2;
     g.Vh = g.Xh * g.Y * g.Z * g.T;
+    g.ntiles = (g.Vh + TILE - 1) / TILE;
     g.sy = g.Xh; g.sz = g.Xh * g.Y; g.st = g.Xh * g.Y * g.Z;
     c->complex_bc = cbc;
     c->block = 64;
-    c->depth = 0;
     *ctx = c;
     return LQCD_OK;
 }
@@ -170,7 +146,9 @@ lqcd_status lqcd_destroy(lqcd_ctx* ctx) {
 }
 
 size_t lqcd_spinor_bytes(const lqcd_ctx* c, int half) { return c ? half_bytes(c) * (half ? 1 : 2) : 0; }
-size_t lqcd_gauge_bytes(const lqcd_ctx* c) { return c ? (size_t)8 * c->p.recon * c->g.Vh * elem(c) : 0; }
+size_t lqcd_gauge_bytes(const lqcd_ctx* c) {
+    return c ? (size_t)2 * 8 * c->p.recon * TILE * c->g.ntiles * elem(c) : 0;  // [parity][tile][hop 8][recon reals][32]
+}
 size_t lqcd_workspace_bytes(const lqcd_ctx* c) { return c ? half_bytes(c) : 0; }
 
 size_t lqcd_host_workspace_bytes(const lqcd_ctx* c) {
@@ -187,18 +165,10 @@ lqcd_status lqcd_set_block_threads(lqcd_ctx* c, int b) {
     return LQCD_OK;
 }
 
-lqcd_status lqcd_set_link_stage_depth(lqcd_ctx* c, int depth) {
-    if (!c) return LQCD_EINVAL;
-    if (depth < 0) depth = 0;
-    if (depth != 0 && depth != 4 && depth != 8) return LQCD_EINVAL;
-    c->depth = depth;
-    return LQCD_OK;
-}
-
 lqcd_status lqcd_pack_gauge(const lqcd_ctx* c, void* native, const void* canon, void* stream) {
     if (!c || !native || !canon) return LQCD_EINVAL;
     if (!aligned16(native) || !aligned16(canon)) return LQCD_EALIGN;
-    const dim3 grid((c->g.Vh + 127) / 128, 4, 2);
+    const dim3 grid((c->g.Vh + 127) / 128, 8, 2);
     cudaStream_t st = (cudaStream_t)stream;
     if (c->p.precision == 32) {
         if (c->p.recon == 12) pack_gauge_kernel<float, 12><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);

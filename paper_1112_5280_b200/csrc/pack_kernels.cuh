@@ -1,6 +1,6 @@
 // pack_kernels.cuh -- canonical (interchange) <-> native layout conversion (step L0).
 // Layout only, no arithmetic of the method; built once per field, not on the timed path.
-// Layouts are specified in include/lqcd.h.
+// Layouts are specified in include/lqcd.h and fields.cuh.
 #pragma once
 #include "fields.cuh"
 #include "geometry.cuh"
@@ -13,20 +13,32 @@ __device__ __forceinline__ size_t lex_of(const Geom& g, int cb, int p) {
     return (size_t)2 * cb + s.x_odd;
 }
 
-// canonical links [mu][V][3][3] complex -> native [parity][mu][word][Vh][lane], first RECON reals.
+// lex index of the site one step back along mu from (parity p, cb), periodic wrap (links carry no phase)
+__device__ __forceinline__ size_t lex_back(const Geom& g, int cb, int p, int mu) {
+    const Site s = decode_site(g, cb, p);
+    int c[4] = {2 * s.xh + s.x_odd, s.y, s.z, s.t};
+    const int L[4] = {g.X, g.Y, g.Z, g.T};
+    c[mu] = c[mu] == 0 ? L[mu] - 1 : c[mu] - 1;
+    return (size_t)c[0] + (size_t)g.X * (c[1] + (size_t)g.Y * (c[2] + (size_t)g.Z * c[3]));
+}
+
+// canonical links [mu][V][3][3] complex -> native, gathered by output site (fields.cuh): for site cb of
+// parity p, hop k = 2 mu holds U_mu(x), hop k = 2 mu + 1 holds U_mu(x - mu^); first RECON reals of each.
+// grid: (ceil(Vh / block), 8 hops, 2 parities).
 template <typename R, int RECON>
 __global__ void pack_gauge_kernel(R* __restrict__ native, const R* __restrict__ canon, Geom g) {
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= g.Vh) return;
-    const int mu = blockIdx.y, p = blockIdx.z;
+    const int k = blockIdx.y, p = blockIdx.z, mu = k >> 1;
     constexpr int LW = LinkWord<R, RECON>::LW, NW = RECON / LW;
     const size_t V = (size_t)2 * g.Vh;
-    const R* src = canon + ((size_t)mu * V + lex_of(g, cb, p)) * 18;
-    R* dst = native + ((size_t)((p * 4 + mu) * NW) * g.Vh + cb) * LW;
+    const size_t site = (k & 1) ? lex_back(g, cb, p, mu) : lex_of(g, cb, p);
+    const R* src = canon + ((size_t)mu * V + site) * 18;
+    R* dst = native + link_word0<R, RECON>(g.ntiles, p, cb, k) * LW;
 #pragma unroll
     for (int w = 0; w < NW; ++w)
 #pragma unroll
-        for (int l = 0; l < LW; ++l) dst[(size_t)w * g.Vh * LW + l] = src[w * LW + l];
+        for (int l = 0; l < LW; ++l) dst[(size_t)w * TILE * LW + l] = src[w * LW + l];
 }
 
 // mode 0/1: canonical half spinor [Vh][4][3] of that parity <-> native half spinor.
@@ -42,22 +54,23 @@ __global__ void pack_spinor_kernel(R* __restrict__ dst_, const R* __restrict__ s
     } else {
         const int p = blockIdx.y;
         canon_site = lex_of(g, cb, p);
-        native_off = (size_t)p * 24 * g.Vh;
+        native_off = (size_t)p * 24 * TILE * g.ntiles;
     }
+    const size_t w0 = spinor_word0<R>(cb) * W;
     if (UNPACK) {
-        const R* nat = src_ + native_off;
+        const R* nat = src_ + native_off + w0;
         R* can = dst_ + canon_site * 24;
 #pragma unroll
         for (int q = 0; q < Q; ++q)
 #pragma unroll
-            for (int l = 0; l < W; ++l) can[q * W + l] = nat[((size_t)q * g.Vh + cb) * W + l];
+            for (int l = 0; l < W; ++l) can[q * W + l] = nat[(size_t)q * TILE * W + l];
     } else {
-        R* nat = dst_ + native_off;
+        R* nat = dst_ + native_off + w0;
         const R* can = src_ + canon_site * 24;
 #pragma unroll
         for (int q = 0; q < Q; ++q)
 #pragma unroll
-            for (int l = 0; l < W; ++l) nat[((size_t)q * g.Vh + cb) * W + l] = can[q * W + l];
+            for (int l = 0; l < W; ++l) nat[(size_t)q * TILE * W + l] = can[q * W + l];
     }
 }
 

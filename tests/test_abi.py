@@ -34,10 +34,12 @@ def test_create_validation_and_sizes():
     assert c.Vh == Vh
     assert c.spinor_bytes(True) == Vh * 24 * 4
     assert c.spinor_bytes(False) == Vh * 48 * 4
-    assert c.gauge_bytes() == 8 * 12 * Vh * 4
+    assert c.gauge_bytes() == 2 * 8 * 12 * Vh * 4  # gathered by output site: every link stored twice
     assert c.workspace_bytes() == Vh * 24 * 4
     c = L.Context((4, 4, 4, 4), 64, 18)
-    assert c.gauge_bytes() == 8 * 18 * 128 * 8
+    assert c.gauge_bytes() == 2 * 8 * 18 * 128 * 8
+    c6 = L.Context((6, 6, 6, 6), 32, 12)  # Vh = 648 is padded to 21 tiles of 32 sites
+    assert c6.spinor_bytes(True) == 21 * 32 * 24 * 4 and c6.gauge_bytes() == 2 * 21 * 32 * 8 * 12 * 4
     assert c.host_workspace_bytes() >= c.gauge_bytes() + 4 * 256 * 18 * 8 + 4 * c.spinor_bytes(True)
     for bad in [dict(dims=(4, 4, 3, 4)), dict(dims=(2, 4, 4, 4)), dict(precision=16), dict(recon=8),
                 dict(bc=(1, 1, 1, 0.5))]:
@@ -49,9 +51,6 @@ def test_create_validation_and_sizes():
     c.set_block_threads(128)
     with pytest.raises(L.LqcdError):
         c.set_block_threads(100)
-    c.set_link_stage_depth(8)
-    with pytest.raises(L.LqcdError):
-        c.set_link_stage_depth(3)
 
 
 def test_null_pointers_rejected_without_gpu():

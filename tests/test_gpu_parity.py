@@ -117,9 +117,8 @@ def test_ragged_anisotropic_complex_bc(H, precision, recon):
     U = li.random_su3_links(dims, seed=21).astype(cdtype(precision))
     psi = li.gaussian_spinor(dims, seed=22).astype(cdtype(precision))
     g = H.Gpu(dims, precision, recon, bc, U)
-    for blk, depth in ((64, 0), (128, 0), (64, 4), (128, 4), (64, 8), (128, 8)):
+    for blk in (64, 128):
         g.ctx.set_block_threads(blk)
-        g.ctx.set_link_stage_depth(depth)
         assert H.rel_l2(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc)) <= TOL[precision]
         for op in (0, 1):
             ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, op), dims, op)
