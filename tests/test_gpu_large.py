@@ -75,16 +75,21 @@ def test_config4_full_field_fp32_vs_oracle(cfg4):
     assert H.rel_l2(g.dslash_eo(H.half_of(psi, dims, 1), 0), ref) <= TOL[32]
 
 
+@pytest.fixture(scope="module")
+def cfg5():
+    """Config-5 inputs, generated once for both link-storage variants (the A11 link field takes minutes)."""
+    c = li.CONFIGS[5]
+    return c, li.links_for_config(5, dtype=np.complex64), li.gaussian_spinor(c["dims"], dtype=np.complex64)
+
+
 @pytest.mark.parametrize("recon", [12, 18])
-def test_config5_chain_per_step_parity(recon):
+def test_config5_chain_per_step_parity(cfg5, recon):
     """Config 5 (reading A16): x_{k+1} = M x_k chained 100 times in fp32; per-step parity at
     k in {1, 50, 100}: the oracle is fed the GPU's own x_k and compared with x_{k+1} at sampled sites."""
     import torch
     import gpu_harness as H
-    c = li.CONFIGS[5]
+    c, U, psi = cfg5
     dims, bc, kappa = c["dims"], c["bc"], c["kappa"]
-    U = li.links_for_config(5, dtype=np.complex64)
-    psi = li.gaussian_spinor(dims, dtype=np.complex64)
     g = H.Gpu(dims, 32, recon, bc, U)
     x = g.to_native(H.half_of(psi, dims, 0), 0)
     y, ws = g.buf(), g.buf()
