@@ -134,7 +134,7 @@ class ClockSampler:
 class Workload:
     """Seeded inputs of one config on the device in native layout, plus pinned host copies."""
 
-    def __init__(self, cfg_id, precision, recon, dev, block=0, nbuf=NBUF, keep_host=True, in_parity=None):
+    def __init__(self, cfg_id, precision, recon, dev, block=0, nbuf=NBUF, keep_host=True, in_parity=None, U=None):
         import numpy as np
         import torch
         import lattice_inputs as li
@@ -148,7 +148,8 @@ class Workload:
         if block:
             self.ctx.set_block_threads(block)
         self.Vh = self.ctx.Vh
-        U = li.links_for_config(cfg_id, dtype=cd)
+        if U is None:
+            U = li.links_for_config(cfg_id, dtype=cd)
         self.U_host = torch.from_numpy(U).pin_memory() if keep_host else None
         self.gauge = torch.empty(self.ctx.gauge_bytes(), dtype=torch.uint8, device=dev)
         Ud = torch.from_numpy(U).to(dev)
@@ -266,10 +267,10 @@ def e2e_leg(torch, w, steps, world):
     }
 
 
-def chain_leg(torch, cfg_id, precision, recon, dev, napply=100, reps=3):
+def chain_leg(torch, cfg_id, precision, recon, dev, napply=100, reps=3, U=None):
     """Config 5 (reading A16): x_{k+1} = M x_k, M = 1 - kappa^2 H_eo H_oe, `napply` times back to back,
     ping-pong buffers, timed as one block."""
-    w = Workload(cfg_id, precision, recon, dev, nbuf=1, keep_host=False, in_parity=0)  # even half spinor
+    w = Workload(cfg_id, precision, recon, dev, nbuf=1, keep_host=False, in_parity=0, U=U)  # even half spinor
     x, y = w.inp[0], w.out[0]
     ws = torch.empty_like(x)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -400,7 +401,11 @@ def run_b200(args):
         torch.cuda.empty_cache()
         if rank == 0:
             if args.chain:  # config 5; opt-in: generating its 3 GB A11 link field takes minutes of host time
-                line["chain"] = [chain_leg(torch, 5, 32, rc, dev) for rc in (12, 18)]
+                import numpy as np
+                import lattice_inputs as li
+                U5 = li.links_for_config(5, dtype=np.complex64)
+                line["chain"] = [chain_leg(torch, 5, 32, rc, dev, U=U5) for rc in (12, 18)]
+                del U5
             line["cpu_baseline"] = cpu_baseline_leg(args.config, args.precision)
     if dist is not None:
         dist.barrier()
