@@ -199,12 +199,21 @@ def timed_steps(torch, dist, fn, steps, warmup):
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
-    ms = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    return ms
+    return max_over_ranks(torch, dist, e0.elapsed_time(e1), "cuda")
+
+
+def max_over_ranks(torch, dist, ms, device):
+    """Multi-GPU timing rule: the time of a replicated run is the slowest rank's device time."""
+    if dist is None:
+        return float(ms)
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_gflops(world, sites_per_step_per_rank, ms_per_step):
+    """Whole-job throughput of `world` independent replicas (weak scaling, no data-path collective)."""
+    return world * sites_per_step_per_rank * FLOP_PER_SITE / (ms_per_step * 1e-3) / 1e9
 
 
 def kernel_leg(torch, dist, w, steps, warmup, world):
@@ -218,7 +227,7 @@ def kernel_leg(torch, dist, w, steps, warmup, world):
     return {
         "ms_per_step": ms_step,
         "us_per_launch": t_launch * 1e6,
-        "gflops": world * w.sites_per_step() * FLOP_PER_SITE / (ms_step * 1e-3) / 1e9,
+        "gflops": aggregate_gflops(world, w.sites_per_step(), ms_step),
         "gbs": w.bytes_per_launch() / t_launch / 1e9,
         "launches": launches,
     }
