@@ -50,6 +50,7 @@ def _load():
         lib.oracle_dslash_full.argtypes = common
         lib.oracle_dslash_eo.argtypes = common + [c_int]
         lib.oracle_apply_M.argtypes = common + [c_dbl, c_int]
+        lib.oracle_apply_M_tm.argtypes = common + [c_dbl, c_dbl, c_int]
         lib.oracle_dslash_sites.argtypes = common + [c_void, c_long]
         lib.oracle_apply_M_sites.argtypes = common + [c_dbl, c_int, c_void, c_long]
         lib.oracle_recon_row2.argtypes = [c_void, c_void, c_void]
@@ -119,6 +120,16 @@ def apply_M(U, psi, dims, bc, kappa: float, eo: int) -> np.ndarray:
     out = np.empty(psi.shape, dtype=np.complex128)
     _check(_load().oracle_apply_M(_ptr(out), _ptr(U), uf, _ptr(psi), pf, _ptr(d), _ptr(bre), _ptr(bim),
                                   float(kappa), int(eo)))
+    return out
+
+
+def apply_M_tm(U, psi, dims, bc, kappa: float, mu: float, eo: int) -> np.ndarray:
+    """Twisted-mass fermion matrix (next row f1).  eo=0: (1 + 2i kappa mu g5) psi - kappa H psi.
+    eo=1: (1 + 2i kappa mu g5) psi_e - kappa^2 H_eo (1 + 2i kappa mu g5)^-1 H_oe psi_e on even sites, zero on odd."""
+    U, uf, psi, pf, d, bre, bim = _prep(U, psi, dims, bc)
+    out = np.empty(psi.shape, dtype=np.complex128)
+    _check(_load().oracle_apply_M_tm(_ptr(out), _ptr(U), uf, _ptr(psi), pf, _ptr(d), _ptr(bre), _ptr(bim),
+                                     float(kappa), float(mu), int(eo)))
     return out
 
 

@@ -38,7 +38,9 @@
  * spectrum on 4^4 (dense matrix), P3 gamma5-hermiticity, P4 even-odd == full,
  * P5 gauge covariance, P6 constant field, P7 point source written out by hand,
  * P8 Clifford algebra / projectors, P9 two-row reconstruction, P10 independent
- * numpy.roll formulation (oracle/roll_formulation.py), P11 linearity/translation.
+ * numpy.roll formulation (oracle/roll_formulation.py), P11 linearity/translation; twisted-mass operator
+ * (next row f1): T1 mu = 0 reduces to apply_M, T2 free-field plane waves, T3 gamma5 M(mu) gamma5 = M(-mu)^dagger,
+ * T4 even-odd form = Schur complement of the full operator.
  * Parity unpinned: nothing.
  */
 #include <complex.h>
@@ -273,6 +275,106 @@ int oracle_apply_M(double complex *out, const void *U, int u_f32, const void *ps
         }
     }
     free(tmp);
+    return 0;
+}
+
+/* ---- next row f1: twisted-mass Wilson fermions ("N_f = 2 twisted-mass Wilson fermions [18, 21]",
+ * "even-odd preconditioning"; the paper prints no formula -- DESIGN.md reading F1) -------------------------
+ *   M_tm(mu)     = (1 + 2 i kappa mu gamma_5) - kappa H                         (one flavour; the other has -mu)
+ *   Mhat_tm(mu)  = (1 + 2 i kappa mu gamma_5) - kappa^2 H_eo (1 + 2 i kappa mu gamma_5)^-1 H_oe   on even sites
+ * i.e. the Schur complement of M_tm with respect to the odd sites.  The site-diagonal matrix and its inverse
+ * are built as dense 4x4 complex matrices; the inverse by Gauss-Jordan elimination, not by the closed form. */
+static void tm_diag(cplx d[4][4], double theta) {
+    for (int s = 0; s < 4; ++s)
+        for (int t = 0; t < 4; ++t) d[s][t] = (s == t ? 1.0 : 0.0) + I * theta * GAMMA[4][s][t];
+}
+
+static int inv4(cplx inv[4][4], cplx a[4][4]) {
+    cplx m[4][8];
+    for (int r = 0; r < 4; ++r)
+        for (int c = 0; c < 8; ++c) m[r][c] = c < 4 ? a[r][c] : (c - 4 == r ? 1.0 : 0.0);
+    for (int col = 0; col < 4; ++col) {
+        int piv = col;
+        for (int r = col + 1; r < 4; ++r)
+            if (cabs(m[r][col]) > cabs(m[piv][col])) piv = r;
+        if (cabs(m[piv][col]) == 0.0) return 1;
+        for (int c = 0; c < 8; ++c) { cplx t = m[col][c]; m[col][c] = m[piv][c]; m[piv][c] = t; }
+        cplx d = m[col][col];
+        for (int c = 0; c < 8; ++c) m[col][c] /= d;
+        for (int r = 0; r < 4; ++r)
+            if (r != col) {
+                cplx fct = m[r][col];
+                for (int c = 0; c < 8; ++c) m[r][c] -= fct * m[col][c];
+            }
+    }
+    for (int r = 0; r < 4; ++r)
+        for (int c = 0; c < 4; ++c) inv[r][c] = m[r][c + 4];
+    return 0;
+}
+
+/* v <- d v for every site of the field (12 complex per site, spin-major) */
+static void spin_mul_field(cplx *v, size_t nsites, cplx d[4][4]) {
+#pragma omp parallel for schedule(static)
+    for (long n = 0; n < (long)nsites; ++n) {
+        cplx t[4][3];
+        for (int s = 0; s < 4; ++s)
+            for (int a = 0; a < 3; ++a) {
+                cplx acc = 0;
+                for (int sp = 0; sp < 4; ++sp) acc += d[s][sp] * v[(size_t)n * 12 + sp * 3 + a];
+                t[s][a] = acc;
+            }
+        for (int s = 0; s < 4; ++s)
+            for (int a = 0; a < 3; ++a) v[(size_t)n * 12 + s * 3 + a] = t[s][a];
+    }
+}
+
+/* eo = 0: out = (1 + 2 i kappa mu g5) psi - kappa H psi on all sites.
+ * eo = 1: out_e = (1 + 2 i kappa mu g5) psi_e - kappa^2 H_eo (1 + 2 i kappa mu g5)^-1 H_oe psi_e, zero on odd sites. */
+int oracle_apply_M_tm(double complex *out, const void *U, int u_f32, const void *psi, int psi_f32,
+                      const int dims[4], const double bc_re[4], const double bc_im[4], double kappa, double mu,
+                      int eo) {
+    fields_t f;
+    if (!out || setup(&f, U, u_f32, psi, psi_f32, dims, bc_re, bc_im)) return 1;
+    if (eo != 0 && eo != 1) return 1;
+    const size_t nsites = (size_t)dims[0] * dims[1] * dims[2] * dims[3], n = nsites * 12;
+    cplx d[4][4], dinv[4][4];
+    tm_diag(d, 2.0 * kappa * mu);
+    if (inv4(dinv, d)) return 3;
+    cplx *diag = (cplx *)malloc(n * sizeof(cplx)); /* (1 + 2 i kappa mu g5) psi */
+    if (!diag) return 2;
+    for (size_t k = 0; k < n; ++k) diag[k] = ld(psi, k, psi_f32);
+    spin_mul_field(diag, nsites, d);
+    if (eo == 0) {
+        hop_field(out, &f, -1);
+        for (size_t k = 0; k < n; ++k) out[k] = diag[k] - kappa * out[k];
+        free(diag);
+        return 0;
+    }
+    for (int m = 0; m < 4; ++m)
+        if (dims[m] & 1) { free(diag); return 1; }
+    cplx *tmp = (cplx *)malloc(n * sizeof(cplx));
+    if (!tmp) { free(diag); return 2; }
+    hop_field(tmp, &f, 1);               /* tmp_o = H_oe psi_e */
+    spin_mul_field(tmp, nsites, dinv);   /* tmp_o = (1 + 2 i kappa mu g5)^-1 tmp_o  (zero stays zero on even sites) */
+    fields_t g = f;
+    g.psi = tmp;
+    g.psi_f32 = 0;
+    hop_field(out, &g, 0);               /* out_e = H_eo tmp_o */
+    const int X = dims[0], Y = dims[1], Z = dims[2];
+    for (size_t site = 0; site < nsites; ++site) {
+        size_t r = site;
+        int x0 = (int)(r % X); r /= X;
+        int x1 = (int)(r % Y); r /= Y;
+        int x2 = (int)(r % Z); r /= Z;
+        int x3 = (int)r;
+        int even = ((x0 + x1 + x2 + x3) & 1) == 0;
+        for (int k = 0; k < 12; ++k) {
+            size_t idx = site * 12 + k;
+            out[idx] = even ? diag[idx] - kappa * kappa * out[idx] : 0;
+        }
+    }
+    free(tmp);
+    free(diag);
     return 0;
 }
 
