@@ -307,6 +307,32 @@ def chain_leg(torch, cfg_id, precision, recon, dev, napply=100, reps=3, U=None):
     }
 
 
+def matrix_leg(torch, w, napply=50, reps=3):
+    """Fermion-matrix applications on the primary workload's fields: lqcd_apply_M(eo=1) and the twisted-mass
+    lqcd_apply_M_tm(eo=1) (next row f1), napply back-to-back applications alternating between two input
+    buffers, best of `reps`.  2 launches, 2 x 1320 flop and (2 x (24 + 24 + 8 recon) + 24) reals per even site."""
+    x, y, ws = w.inp[1], w.out[1], w.out[0]   # inp[1] holds an even half spinor (out_parity 1)
+    x2, y2 = w.inp[3 % w.nbuf], w.out[3 % w.nbuf]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    res = {}
+    for name, fn in (("apply_M", lambda o, i: w.ctx.apply_M(o, w.gauge, i, w.kappa, 1, ws)),
+                     ("apply_M_tm", lambda o, i: w.ctx.apply_M_tm(o, w.gauge, i, w.kappa, 0.05, 1, ws))):
+        best = None
+        for _ in range(reps + 1):
+            torch.cuda.synchronize()
+            e0.record()
+            for k in range(napply):
+                fn(y, x) if k & 1 else fn(y2, x2)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / napply
+            best = ms if best is None else min(best, ms)
+        nbytes = (2 * REALS_PER_SITE[w.recon] + 24) * (w.precision // 8) * w.Vh
+        res[name] = {"us_per_application": best * 1e3, "gflops": 2 * FLOP_PER_SITE * w.Vh / (best * 1e-3) / 1e9,
+                     "gbs": nbytes / (best * 1e-3) / 1e9}
+    return res
+
+
 def cpu_baseline_leg(cfg_id, precision):
     """The oracle as it stands on the host cores: full-lattice dslash_eo of the same workload,
     one warm-up then best of 3 (about 2-5 s of CPU work on 8+ cores)."""
@@ -396,6 +422,7 @@ def run_b200(args):
     }
 
     if not args.no_extras and rank == 0:
+        line["matrix"] = matrix_leg(torch, w)
         line["e2e"] = e2e_leg(torch, w, max(1, min(args.steps, 10)), 1)
     del w
     torch.cuda.empty_cache()

@@ -117,6 +117,16 @@ lqcd_status lqcd_dslash_eo(const lqcd_ctx* ctx, void* out_dev, const void* gauge
 lqcd_status lqcd_apply_M(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
                          double kappa, int eo, void* workspace_dev, void* stream);
 
+/* Twisted-mass Wilson fermion matrix for one flavour ("N_f = 2 twisted-mass Wilson fermions",
+ * "even-odd preconditioning"; the other flavour is mu -> -mu; reading F1):
+ * eo = 0: out = (1 + 2 i kappa mu gamma_5) in - kappa H in, native full spinors, one launch.
+ * eo = 1: out_e = (1 + 2 i kappa mu gamma_5) in_e - kappa^2 H_eo (1 + 2 i kappa mu gamma_5)^-1 H_oe in_e, the Schur
+ *         complement on the even sites; native even half spinors; two launches; workspace as for lqcd_apply_M.
+ * The site-diagonal term and its inverse are applied in the epilogues of the dslash launches (gamma_5 is
+ * diagonal in the chiral basis), so the traffic is that of lqcd_apply_M.  mu = 0 gives lqcd_apply_M. */
+lqcd_status lqcd_apply_M_tm(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
+                            double kappa, double mu, int eo, void* workspace_dev, void* stream);
+
 /* End-to-end convenience for host-resident data: canonical host buffers in, canonical host
  * buffer out.  Copies gauge_host (canonical links; may be NULL to reuse the links packed into
  * workspace_dev by an earlier call) and in_host (canonical half spinor of parity 1-out_parity)

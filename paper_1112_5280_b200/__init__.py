@@ -18,7 +18,7 @@ PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, -1
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
-    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_dslash_eo_host", "lqcd_launch_count",
+    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_apply_M_tm", "lqcd_dslash_eo_host", "lqcd_launch_count",
     "lqcd_set_block_threads", "lqcd_status_string", "lqcd_last_cuda_error",
 ]
 
@@ -62,6 +62,7 @@ def _lib():
         lib.lqcd_dslash_full.argtypes = [vp, vp, vp, vp, vp]
         lib.lqcd_dslash_eo.argtypes = [vp, vp, vp, vp, ci, vp]
         lib.lqcd_apply_M.argtypes = [vp, vp, vp, vp, cd, ci, vp, vp]
+        lib.lqcd_apply_M_tm.argtypes = [vp, vp, vp, vp, cd, cd, ci, vp, vp]
         lib.lqcd_dslash_eo_host.argtypes = [vp, vp, vp, vp, ci, vp, vp]
         lib.lqcd_launch_count.argtypes = []
         lib.lqcd_launch_count.restype = ctypes.c_ulonglong
@@ -149,6 +150,10 @@ class Context:
     def apply_M(self, out, gauge, inp, kappa, eo, workspace=None, stream=None):
         _chk(_lib().lqcd_apply_M(self._h, _ptr(out), _ptr(gauge), _ptr(inp), float(kappa), int(eo),
                                  _ptr(workspace), _stream(stream)), "lqcd_apply_M")
+
+    def apply_M_tm(self, out, gauge, inp, kappa, mu, eo, workspace=None, stream=None):
+        _chk(_lib().lqcd_apply_M_tm(self._h, _ptr(out), _ptr(gauge), _ptr(inp), float(kappa), float(mu), int(eo),
+                                    _ptr(workspace), _stream(stream)), "lqcd_apply_M_tm")
 
     def dslash_eo_host(self, out_host, gauge_host, in_host, out_parity, workspace, stream=None):
         _chk(_lib().lqcd_dslash_eo_host(self._h, _ptr(out_host), _ptr(gauge_host), _ptr(in_host), int(out_parity),

@@ -161,14 +161,35 @@ template <> struct MinBlocks<float, 18>  { static constexpr int value = LQCD_MIN
 template <> struct MinBlocks<double, 12> { static constexpr int value = LQCD_MINB_F64_R12; };
 template <> struct MinBlocks<double, 18> { static constexpr int value = LQCD_MINB_F64_R18; };
 
-// out_p(x) = (H in)(x)              (XPAY = false)
-// out_p(x) = xin(x) + a (H in)(x)    (XPAY = true; a = -kappa or -kappa^2, step K6)
+// Step K6, the epilogue applied to acc = (H in)(x) before the store (EPI):
+//   EPI_STORE    out = acc                                        lqcd_dslash_*
+//   EPI_XPAY     out = x + a acc                                  lqcd_apply_M   (a = -kappa or -kappa^2)
+//   EPI_G5SCALE  out = (g_re + i g_im gamma_5) acc                lqcd_apply_M_tm, first pass: (1 + i theta g5)^-1 H_oe in
+//   EPI_G5XPAY   out = (g_re + i g_im gamma_5) x + a acc          lqcd_apply_M_tm, last pass:  (1 + i theta g5) in - kappa^2 H ...
+// gamma_5 = diag(1, 1, -1, -1) in the chiral basis, so the twisted-mass site-diagonal term is a complex
+// scalar on the upper two spin components and its conjugate on the lower two: it costs no extra memory traffic.
+enum { EPI_STORE = 0, EPI_XPAY = 1, EPI_G5SCALE = 2, EPI_G5XPAY = 3 };
+template <typename R> struct Epilogue { R a, g_re, g_im; };
+
+// v <- (g_re + i g_im gamma_5) v
+template <typename R>
+__device__ __forceinline__ void g5_scale(R v[24], R g_re, R g_im) {
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+        const R gi = k < 6 ? g_im : -g_im;
+        const R re = v[2 * k], im = v[2 * k + 1];
+        v[2 * k] = fma_(-gi, im, g_re * re);
+        v[2 * k + 1] = fma_(gi, re, g_re * im);
+    }
+}
+
 // grid.y = 1: one parity `parity0`; grid.y = 2: both, parity = blockIdx.y, and in/out/xin are
 // full fields [even|odd] (in is read at the opposite half).  One thread per output site.
-template <typename R, int RECON, bool XPAY, bool CBC, int BLOCK>
+template <typename R, int RECON, int EPI, bool CBC, int BLOCK>
 __global__ void __launch_bounds__(BLOCK, MinBlocks<R, RECON>::value * 64 / BLOCK)
 dslash_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __restrict__ in,
-              const R* __restrict__ xin, R a, Geom g, int parity0, BcPhases<R> bc) {
+              const R* __restrict__ xin, Epilogue<R> epi, Geom g, int parity0, BcPhases<R> bc) {
+    constexpr bool XPAY = EPI == EPI_XPAY || EPI == EPI_G5XPAY;
     int p = parity0;
     if (gridDim.y == 2) {
         p = blockIdx.y;
@@ -211,11 +232,13 @@ dslash_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __restr
     hop_step<R, RECON, CBC, 6>(acc, site_links, in, nb, crossmask, bc);
     hop_step<R, RECON, CBC, 7>(acc, site_links, in, nb, crossmask, bc);
 
-    if (XPAY) {
+    if constexpr (EPI == EPI_G5SCALE) g5_scale<R>(acc, epi.g_re, epi.g_im);
+    if constexpr (XPAY) {
         R x[24];
         load_spinor<R>(xin, cb, x);
+        if constexpr (EPI == EPI_G5XPAY) g5_scale<R>(x, epi.g_re, epi.g_im);
 #pragma unroll
-        for (int k = 0; k < 24; ++k) acc[k] = fma_(a, acc[k], x[k]);
+        for (int k = 0; k < 24; ++k) acc[k] = fma_(epi.a, acc[k], x[k]);
     }
     store_spinor<R>(out, cb, acc);
 }

@@ -58,45 +58,57 @@ BcPhases<R> make_bc(const lqcd_ctx* c) {
     return b;
 }
 
-template <typename R, int RECON, bool XPAY, bool CBC, int BLOCK>
+// epilogue of one launch: mode (EPI_*) and its constants, in double until the kernel's precision is known
+struct EpiArgs { int mode; double a, g_re, g_im; };
+
+template <typename R, int RECON, int EPI, bool CBC, int BLOCK>
 lqcd_status launch_block(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                         double a, int parity, cudaStream_t st) {
+                         const EpiArgs& e, int parity, cudaStream_t st) {
     const dim3 grid((c->g.Vh + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
-    dslash_kernel<R, RECON, XPAY, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
-        (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, (R)a, c->g, parity < 0 ? 0 : parity, make_bc<R>(c));
+    const Epilogue<R> epi{(R)e.a, (R)e.g_re, (R)e.g_im};
+    dslash_kernel<R, RECON, EPI, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
+        (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<R>(c));
     return after_launch();
 }
 
-template <typename R, int RECON, bool XPAY, bool CBC>
+template <typename R, int RECON, int EPI, bool CBC>
 lqcd_status launch_cbc(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                       double a, int parity, cudaStream_t st) {
+                       const EpiArgs& e, int parity, cudaStream_t st) {
     switch (c->block) {
-        case 64: return launch_block<R, RECON, XPAY, CBC, 64>(c, out, gauge, in, xin, a, parity, st);
-        case 128: return launch_block<R, RECON, XPAY, CBC, 128>(c, out, gauge, in, xin, a, parity, st);
+        case 64: return launch_block<R, RECON, EPI, CBC, 64>(c, out, gauge, in, xin, e, parity, st);
+        case 128: return launch_block<R, RECON, EPI, CBC, 128>(c, out, gauge, in, xin, e, parity, st);
     }
     return LQCD_EUNSUPPORTED;
 }
 
-template <typename R, int RECON>
-lqcd_status launch_recon(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                         double a, int parity, cudaStream_t st) {
-    if (xin) {
-        return c->complex_bc ? launch_cbc<R, RECON, true, true>(c, out, gauge, in, xin, a, parity, st)
-                             : launch_cbc<R, RECON, true, false>(c, out, gauge, in, xin, a, parity, st);
-    }
-    return c->complex_bc ? launch_cbc<R, RECON, false, true>(c, out, gauge, in, xin, a, parity, st)
-                         : launch_cbc<R, RECON, false, false>(c, out, gauge, in, xin, a, parity, st);
+template <typename R, int RECON, int EPI>
+lqcd_status launch_epi(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                       const EpiArgs& e, int parity, cudaStream_t st) {
+    return c->complex_bc ? launch_cbc<R, RECON, EPI, true>(c, out, gauge, in, xin, e, parity, st)
+                         : launch_cbc<R, RECON, EPI, false>(c, out, gauge, in, xin, e, parity, st);
 }
 
-// out_p = H in (xin == NULL) or xin + a H in.  parity < 0: both parities, full fields.
-lqcd_status launch_dslash(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                          double a, int parity, cudaStream_t st) {
-    if (c->p.precision == 32) {
-        return c->p.recon == 12 ? launch_recon<float, 12>(c, out, gauge, in, xin, a, parity, st)
-                                : launch_recon<float, 18>(c, out, gauge, in, xin, a, parity, st);
+template <typename R, int RECON>
+lqcd_status launch_recon(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                         const EpiArgs& e, int parity, cudaStream_t st) {
+    switch (e.mode) {
+        case EPI_STORE: return launch_epi<R, RECON, EPI_STORE>(c, out, gauge, in, xin, e, parity, st);
+        case EPI_XPAY: return launch_epi<R, RECON, EPI_XPAY>(c, out, gauge, in, xin, e, parity, st);
+        case EPI_G5SCALE: return launch_epi<R, RECON, EPI_G5SCALE>(c, out, gauge, in, xin, e, parity, st);
+        case EPI_G5XPAY: return launch_epi<R, RECON, EPI_G5XPAY>(c, out, gauge, in, xin, e, parity, st);
     }
-    return c->p.recon == 12 ? launch_recon<double, 12>(c, out, gauge, in, xin, a, parity, st)
-                            : launch_recon<double, 18>(c, out, gauge, in, xin, a, parity, st);
+    return LQCD_EUNSUPPORTED;
+}
+
+// out_p = epilogue(H in); parity < 0: both parities, full fields.
+lqcd_status launch_dslash(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                          const EpiArgs& e, int parity, cudaStream_t st) {
+    if (c->p.precision == 32) {
+        return c->p.recon == 12 ? launch_recon<float, 12>(c, out, gauge, in, xin, e, parity, st)
+                                : launch_recon<float, 18>(c, out, gauge, in, xin, e, parity, st);
+    }
+    return c->p.recon == 12 ? launch_recon<double, 12>(c, out, gauge, in, xin, e, parity, st)
+                            : launch_recon<double, 18>(c, out, gauge, in, xin, e, parity, st);
 }
 
 lqcd_status check_fields(const lqcd_ctx* c, const void* out, const void* gauge, const void* in, size_t nbytes) {
@@ -207,7 +219,7 @@ lqcd_status lqcd_unpack_spinor(const lqcd_ctx* c, void* canon, const void* nativ
 lqcd_status lqcd_dslash_full(const lqcd_ctx* c, void* out, const void* gauge, const void* in, void* stream) {
     lqcd_status s = check_fields(c, out, gauge, in, c ? 2 * half_bytes(c) : 0);
     if (s != LQCD_OK) return s;
-    return launch_dslash(c, out, gauge, in, nullptr, 0.0, -1, (cudaStream_t)stream);
+    return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0}, -1, (cudaStream_t)stream);
 }
 
 lqcd_status lqcd_dslash_eo(const lqcd_ctx* c, void* out, const void* gauge, const void* in, int out_parity,
@@ -215,17 +227,18 @@ lqcd_status lqcd_dslash_eo(const lqcd_ctx* c, void* out, const void* gauge, cons
     if (out_parity != 0 && out_parity != 1) return LQCD_EINVAL;
     lqcd_status s = check_fields(c, out, gauge, in, c ? half_bytes(c) : 0);
     if (s != LQCD_OK) return s;
-    return launch_dslash(c, out, gauge, in, nullptr, 0.0, out_parity, (cudaStream_t)stream);
+    return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0}, out_parity, (cudaStream_t)stream);
 }
 
-lqcd_status lqcd_apply_M(const lqcd_ctx* c, void* out, const void* gauge, const void* in, double kappa, int eo,
-                         void* workspace, void* stream) {
+// Shared body of lqcd_apply_M (theta = 0) and lqcd_apply_M_tm (theta = 2 kappa mu).
+static lqcd_status apply_M_impl(const lqcd_ctx* c, void* out, const void* gauge, const void* in, double kappa,
+                                double theta, bool twisted, int eo, void* workspace, cudaStream_t st) {
     if (eo != 0 && eo != 1) return LQCD_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
+    const EpiArgs last{twisted ? EPI_G5XPAY : EPI_XPAY, eo ? -kappa * kappa : -kappa, 1.0, theta};
     if (eo == 0) {
         lqcd_status s = check_fields(c, out, gauge, in, c ? 2 * half_bytes(c) : 0);
         if (s != LQCD_OK) return s;
-        return launch_dslash(c, out, gauge, in, in, -kappa, -1, st);  // out = in - kappa H in
+        return launch_dslash(c, out, gauge, in, in, last, -1, st);  // out = (1 + i theta g5) in - kappa H in
     }
     const size_t hb = c ? half_bytes(c) : 0;
     lqcd_status s = check_fields(c, out, gauge, in, hb);
@@ -233,9 +246,22 @@ lqcd_status lqcd_apply_M(const lqcd_ctx* c, void* out, const void* gauge, const 
     if (!workspace) return LQCD_EINVAL;
     if (!aligned16(workspace)) return LQCD_EALIGN;
     if (overlaps(workspace, hb, in, hb) || overlaps(workspace, hb, out, hb)) return LQCD_EALIAS;
-    s = launch_dslash(c, workspace, gauge, in, nullptr, 0.0, 1, st);  // tmp_o = H_oe in_e
+    // tmp_o = (1 + i theta g5)^-1 H_oe in_e, with (1 + i theta g5)^-1 = (1 - i theta g5) / (1 + theta^2)
+    const double n = 1.0 / (1.0 + theta * theta);
+    const EpiArgs first{twisted ? EPI_G5SCALE : EPI_STORE, 0.0, n, -theta * n};
+    s = launch_dslash(c, workspace, gauge, in, nullptr, first, 1, st);
     if (s != LQCD_OK) return s;
-    return launch_dslash(c, out, gauge, workspace, in, -kappa * kappa, 0, st);  // out_e = in_e - k^2 H_eo tmp_o
+    return launch_dslash(c, out, gauge, workspace, in, last, 0, st);  // out_e = (1 + i theta g5) in_e - kappa^2 H_eo tmp_o
+}
+
+lqcd_status lqcd_apply_M(const lqcd_ctx* c, void* out, const void* gauge, const void* in, double kappa, int eo,
+                         void* workspace, void* stream) {
+    return apply_M_impl(c, out, gauge, in, kappa, 0.0, false, eo, workspace, (cudaStream_t)stream);
+}
+
+lqcd_status lqcd_apply_M_tm(const lqcd_ctx* c, void* out, const void* gauge, const void* in, double kappa, double mu,
+                            int eo, void* workspace, void* stream) {
+    return apply_M_impl(c, out, gauge, in, kappa, 2.0 * kappa * mu, true, eo, workspace, (cudaStream_t)stream);
 }
 
 lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* c, void* out_host, const void* gauge_host, const void* in_host,

@@ -72,13 +72,19 @@ class Gpu:
         self.ctx.dslash_eo(out, self.gauge, self.to_native(psi_half, 1 - out_parity), out_parity)
         return self.from_native(out, out_parity)
 
-    def apply_M(self, psi, kappa, eo):
+    def apply_M(self, psi, kappa, eo, mu=None):
+        """mu = None: lqcd_apply_M; otherwise lqcd_apply_M_tm with twisted mass mu."""
+        def call(out, inp, ws):
+            if mu is None:
+                self.ctx.apply_M(out, self.gauge, inp, kappa, eo, ws)
+            else:
+                self.ctx.apply_M_tm(out, self.gauge, inp, kappa, mu, eo, ws)
         if eo:
             out, ws = self.buf(), self.buf()
-            self.ctx.apply_M(out, self.gauge, self.to_native(psi, 0), kappa, 1, ws)
+            call(out, self.to_native(psi, 0), ws)
             return self.from_native(out, 0)
         out = self.buf(half=False)
-        self.ctx.apply_M(out, self.gauge, self.to_native(psi, -1), kappa, 0, None)
+        call(out, self.to_native(psi, -1), None)
         return self.from_native(out, -1)
 
 

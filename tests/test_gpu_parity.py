@@ -171,3 +171,26 @@ def test_error_codes(H):
         g.ctx.apply_M(a, g.gauge, b, 0.1, 1, b)
     assert e.value.status == L.LQCD_EALIAS
     torch.cuda.synchronize()
+
+
+# ------------------------------------------------------------------ next row f1: twisted-mass matrix
+@pytest.mark.parametrize("precision,recon", [(64, 18), (64, 12), (32, 12), (32, 18)])
+def test_twisted_mass_matrix(H, precision, recon):
+    """lqcd_apply_M_tm against oracle.apply_M_tm: full and even-odd (Schur complement) form, both signs of mu,
+    on configs 2 (random SU(3)) and the ragged anisotropic lattice with complex boundary phases."""
+    from gpu_harness import cdtype
+    cases = [(li.CONFIGS[2]["dims"], li.CONFIGS[2]["bc"], li.links_for_config(2), li.gaussian_spinor(li.CONFIGS[2]["dims"]), 0.15),
+             ((4, 6, 8, 10), np.exp(1j * np.array([0.3, -1.1, 2.0, np.pi])), li.random_su3_links((4, 6, 8, 10), seed=21),
+              li.gaussian_spinor((4, 6, 8, 10), seed=22), 0.13)]
+    for dims, bc, U, psi, kappa in cases:
+        U, psi = U.astype(cdtype(precision)), psi.astype(cdtype(precision))
+        g = H.Gpu(dims, precision, recon, bc, U)
+        for mu in (0.25, -0.4):
+            ref = oracle.apply_M_tm(U, psi, dims, bc, kappa, mu, 0)
+            assert H.rel_l2(g.apply_M(psi, kappa, 0, mu=mu), ref) <= TOL[precision]
+            ref = H.half_of(oracle.apply_M_tm(U, psi, dims, bc, kappa, mu, 1), dims, 0)
+            assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), kappa, 1, mu=mu), ref) <= TOL[precision]
+        # mu = 0 is lqcd_apply_M bit for bit
+        a = g.apply_M(H.half_of(psi, dims, 0), kappa, 1, mu=0.0)
+        b = g.apply_M(H.half_of(psi, dims, 0), kappa, 1)
+        assert H.rel_l2(a, b) <= 1e-15 if precision == 64 else H.rel_l2(a, b) <= 1e-7
