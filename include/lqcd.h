@@ -127,6 +127,25 @@ lqcd_status lqcd_apply_M(const lqcd_ctx* ctx, void* out_dev, const void* gauge_d
 lqcd_status lqcd_apply_M_tm(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
                             double kappa, double mu, int eo, void* workspace_dev, void* stream);
 
+/* Q(mu) = gamma_5 Mhat_tm(mu) on the even sites (even-odd form of lqcd_apply_M_tm with a final gamma_5):
+ * Q(mu)^+ = Q(-mu), so Mhat(mu)^+ Mhat(mu) = Q(-mu) Q(mu).  Native even half spinors, two launches. */
+lqcd_status lqcd_apply_Q_tm(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
+                            double kappa, double mu, void* workspace_dev, void* stream);
+
+/* Conjugate gradient ("the inversion of the fermion matrix"; reading F2): solves
+ *     Mhat_tm(mu)^+ Mhat_tm(mu) x = b      on the even sites, x0 = 0,
+ * textbook CG, stopping when the recursive residual satisfies |r| <= tol |b| or after maxiter iterations.
+ * x_dev, b_dev: native even half spinors (b is not modified; x must not overlap b).  workspace_dev:
+ * lqcd_cg_workspace_bytes(ctx) bytes of device scratch, 256-byte aligned.  All vector updates, reductions and
+ * scalars (alpha, beta, <r,r>, the convergence flag) stay on the device; the host looks at the flag every 8
+ * iterations, and iterations enqueued after convergence leave x untouched.  Reductions are deterministic.
+ * The call synchronises `stream` before returning: *iters_out = iterations performed, *relres_out = |r| / |b|
+ * of the recursive residual (host pointers, either may be NULL).  Arithmetic in the ctx precision. */
+size_t lqcd_cg_workspace_bytes(const lqcd_ctx* ctx);
+lqcd_status lqcd_cg_solve_tm(const lqcd_ctx* ctx, void* x_dev, const void* gauge_dev, const void* b_dev, double kappa,
+                             double mu, double tol, int maxiter, void* workspace_dev, int* iters_out,
+                             double* relres_out, void* stream);
+
 /* End-to-end convenience for host-resident data: canonical host buffers in, canonical host
  * buffer out.  Copies gauge_host (canonical links; may be NULL to reuse the links packed into
  * workspace_dev by an earlier call) and in_host (canonical half spinor of parity 1-out_parity)

@@ -18,7 +18,7 @@ PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, -1
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
-    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_apply_M_tm", "lqcd_dslash_eo_host", "lqcd_launch_count",
+    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_dslash_eo_host", "lqcd_launch_count",
     "lqcd_set_block_threads", "lqcd_status_string", "lqcd_last_cuda_error",
 ]
 
@@ -51,7 +51,7 @@ def _lib():
         vp, ci, cd, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
         lib.lqcd_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(lqcd_params)]
         lib.lqcd_destroy.argtypes = [vp]
-        for n in ("lqcd_gauge_bytes", "lqcd_workspace_bytes", "lqcd_host_workspace_bytes"):
+        for n in ("lqcd_gauge_bytes", "lqcd_workspace_bytes", "lqcd_host_workspace_bytes", "lqcd_cg_workspace_bytes"):
             getattr(lib, n).argtypes = [vp]
             getattr(lib, n).restype = sz
         lib.lqcd_spinor_bytes.argtypes = [vp, ci]
@@ -63,6 +63,8 @@ def _lib():
         lib.lqcd_dslash_eo.argtypes = [vp, vp, vp, vp, ci, vp]
         lib.lqcd_apply_M.argtypes = [vp, vp, vp, vp, cd, ci, vp, vp]
         lib.lqcd_apply_M_tm.argtypes = [vp, vp, vp, vp, cd, cd, ci, vp, vp]
+        lib.lqcd_apply_Q_tm.argtypes = [vp, vp, vp, vp, cd, cd, vp, vp]
+        lib.lqcd_cg_solve_tm.argtypes = [vp, vp, vp, vp, cd, cd, cd, ci, vp, ctypes.POINTER(ci), ctypes.POINTER(cd), vp]
         lib.lqcd_dslash_eo_host.argtypes = [vp, vp, vp, vp, ci, vp, vp]
         lib.lqcd_launch_count.argtypes = []
         lib.lqcd_launch_count.restype = ctypes.c_ulonglong
@@ -123,6 +125,7 @@ class Context:
     def gauge_bytes(self): return _lib().lqcd_gauge_bytes(self._h)
     def workspace_bytes(self): return _lib().lqcd_workspace_bytes(self._h)
     def host_workspace_bytes(self): return _lib().lqcd_host_workspace_bytes(self._h)
+    def cg_workspace_bytes(self): return _lib().lqcd_cg_workspace_bytes(self._h)
 
     def set_block_threads(self, n):
         _chk(_lib().lqcd_set_block_threads(self._h, int(n)), "lqcd_set_block_threads")
@@ -154,6 +157,18 @@ class Context:
     def apply_M_tm(self, out, gauge, inp, kappa, mu, eo, workspace=None, stream=None):
         _chk(_lib().lqcd_apply_M_tm(self._h, _ptr(out), _ptr(gauge), _ptr(inp), float(kappa), float(mu), int(eo),
                                     _ptr(workspace), _stream(stream)), "lqcd_apply_M_tm")
+
+    def apply_Q_tm(self, out, gauge, inp, kappa, mu, workspace, stream=None):
+        _chk(_lib().lqcd_apply_Q_tm(self._h, _ptr(out), _ptr(gauge), _ptr(inp), float(kappa), float(mu),
+                                    _ptr(workspace), _stream(stream)), "lqcd_apply_Q_tm")
+
+    def cg_solve_tm(self, x, gauge, b, kappa, mu, tol, maxiter, workspace, stream=None):
+        """Returns (iterations, |r|/|b|); synchronises the stream."""
+        it, res = ctypes.c_int(0), ctypes.c_double(0.0)
+        _chk(_lib().lqcd_cg_solve_tm(self._h, _ptr(x), _ptr(gauge), _ptr(b), float(kappa), float(mu), float(tol),
+                                     int(maxiter), _ptr(workspace), ctypes.byref(it), ctypes.byref(res),
+                                     _stream(stream)), "lqcd_cg_solve_tm")
+        return it.value, res.value
 
     def dslash_eo_host(self, out_host, gauge_host, in_host, out_parity, workspace, stream=None):
         _chk(_lib().lqcd_dslash_eo_host(self._h, _ptr(out_host), _ptr(gauge_host), _ptr(in_host), int(out_parity),

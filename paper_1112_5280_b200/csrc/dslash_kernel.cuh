@@ -166,10 +166,11 @@ template <> struct MinBlocks<double, 18> { static constexpr int value = LQCD_MIN
 //   EPI_XPAY     out = x + a acc                                  lqcd_apply_M   (a = -kappa or -kappa^2)
 //   EPI_G5SCALE  out = (g_re + i g_im gamma_5) acc                lqcd_apply_M_tm, first pass: (1 + i theta g5)^-1 H_oe in
 //   EPI_G5XPAY   out = (g_re + i g_im gamma_5) x + a acc          lqcd_apply_M_tm, last pass:  (1 + i theta g5) in - kappa^2 H ...
+// With g5_out the stored result is gamma_5 times the above (Q = gamma_5 M, the operator CG works with).
 // gamma_5 = diag(1, 1, -1, -1) in the chiral basis, so the twisted-mass site-diagonal term is a complex
 // scalar on the upper two spin components and its conjugate on the lower two: it costs no extra memory traffic.
 enum { EPI_STORE = 0, EPI_XPAY = 1, EPI_G5SCALE = 2, EPI_G5XPAY = 3 };
-template <typename R> struct Epilogue { R a, g_re, g_im; };
+template <typename R> struct Epilogue { R a, g_re, g_im; int g5_out; };  // g5_out: finally out <- gamma_5 out
 
 // v <- (g_re + i g_im gamma_5) v
 template <typename R>
@@ -239,6 +240,10 @@ dslash_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __restr
         if constexpr (EPI == EPI_G5XPAY) g5_scale<R>(x, epi.g_re, epi.g_im);
 #pragma unroll
         for (int k = 0; k < 24; ++k) acc[k] = fma_(epi.a, acc[k], x[k]);
+    }
+    if (epi.g5_out) {
+#pragma unroll
+        for (int k = 12; k < 24; ++k) acc[k] = -acc[k];
     }
     store_spinor<R>(out, cb, acc);
 }

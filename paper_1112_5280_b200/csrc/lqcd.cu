@@ -9,6 +9,7 @@
 #include <cstring>
 #include <new>
 
+#include "blas_kernels.cuh"
 #include "dslash_kernel.cuh"
 #include "pack_kernels.cuh"
 
@@ -59,13 +60,13 @@ BcPhases<R> make_bc(const lqcd_ctx* c) {
 }
 
 // epilogue of one launch: mode (EPI_*) and its constants, in double until the kernel's precision is known
-struct EpiArgs { int mode; double a, g_re, g_im; };
+struct EpiArgs { int mode; double a, g_re, g_im; int g5_out; };
 
 template <typename R, int RECON, int EPI, bool CBC, int BLOCK>
 lqcd_status launch_block(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
                          const EpiArgs& e, int parity, cudaStream_t st) {
     const dim3 grid((c->g.Vh + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
-    const Epilogue<R> epi{(R)e.a, (R)e.g_re, (R)e.g_im};
+    const Epilogue<R> epi{(R)e.a, (R)e.g_re, (R)e.g_im, e.g5_out};
     dslash_kernel<R, RECON, EPI, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
         (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<R>(c));
     return after_launch();
@@ -219,7 +220,7 @@ lqcd_status lqcd_unpack_spinor(const lqcd_ctx* c, void* canon, const void* nativ
 lqcd_status lqcd_dslash_full(const lqcd_ctx* c, void* out, const void* gauge, const void* in, void* stream) {
     lqcd_status s = check_fields(c, out, gauge, in, c ? 2 * half_bytes(c) : 0);
     if (s != LQCD_OK) return s;
-    return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0}, -1, (cudaStream_t)stream);
+    return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0, 0}, -1, (cudaStream_t)stream);
 }
 
 lqcd_status lqcd_dslash_eo(const lqcd_ctx* c, void* out, const void* gauge, const void* in, int out_parity,
@@ -227,14 +228,14 @@ lqcd_status lqcd_dslash_eo(const lqcd_ctx* c, void* out, const void* gauge, cons
     if (out_parity != 0 && out_parity != 1) return LQCD_EINVAL;
     lqcd_status s = check_fields(c, out, gauge, in, c ? half_bytes(c) : 0);
     if (s != LQCD_OK) return s;
-    return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0}, out_parity, (cudaStream_t)stream);
+    return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0, 0}, out_parity, (cudaStream_t)stream);
 }
 
 // Shared body of lqcd_apply_M (theta = 0) and lqcd_apply_M_tm (theta = 2 kappa mu).
 static lqcd_status apply_M_impl(const lqcd_ctx* c, void* out, const void* gauge, const void* in, double kappa,
-                                double theta, bool twisted, int eo, void* workspace, cudaStream_t st) {
+                                double theta, bool twisted, int eo, void* workspace, cudaStream_t st, int g5_out = 0) {
     if (eo != 0 && eo != 1) return LQCD_EINVAL;
-    const EpiArgs last{twisted ? EPI_G5XPAY : EPI_XPAY, eo ? -kappa * kappa : -kappa, 1.0, theta};
+    const EpiArgs last{twisted ? EPI_G5XPAY : EPI_XPAY, eo ? -kappa * kappa : -kappa, 1.0, theta, g5_out};
     if (eo == 0) {
         lqcd_status s = check_fields(c, out, gauge, in, c ? 2 * half_bytes(c) : 0);
         if (s != LQCD_OK) return s;
@@ -248,7 +249,7 @@ static lqcd_status apply_M_impl(const lqcd_ctx* c, void* out, const void* gauge,
     if (overlaps(workspace, hb, in, hb) || overlaps(workspace, hb, out, hb)) return LQCD_EALIAS;
     // tmp_o = (1 + i theta g5)^-1 H_oe in_e, with (1 + i theta g5)^-1 = (1 - i theta g5) / (1 + theta^2)
     const double n = 1.0 / (1.0 + theta * theta);
-    const EpiArgs first{twisted ? EPI_G5SCALE : EPI_STORE, 0.0, n, -theta * n};
+    const EpiArgs first{twisted ? EPI_G5SCALE : EPI_STORE, 0.0, n, -theta * n, 0};
     s = launch_dslash(c, workspace, gauge, in, nullptr, first, 1, st);
     if (s != LQCD_OK) return s;
     return launch_dslash(c, out, gauge, workspace, in, last, 0, st);  // out_e = (1 + i theta g5) in_e - kappa^2 H_eo tmp_o
@@ -262,6 +263,115 @@ lqcd_status lqcd_apply_M(const lqcd_ctx* c, void* out, const void* gauge, const 
 lqcd_status lqcd_apply_M_tm(const lqcd_ctx* c, void* out, const void* gauge, const void* in, double kappa, double mu,
                             int eo, void* workspace, void* stream) {
     return apply_M_impl(c, out, gauge, in, kappa, 2.0 * kappa * mu, true, eo, workspace, (cudaStream_t)stream);
+}
+
+// ---- next row f2: CG on the normal equations of the even-odd twisted-mass matrix -------------------------
+// A = Mhat(mu)^+ Mhat(mu) = Q(-mu) Q(mu) with Q(mu) = gamma_5 Mhat(mu)  (gamma_5 Mhat(mu) gamma_5 = Mhat(-mu)^+).
+
+}  // extern "C" (templates below)
+
+namespace {
+
+struct CgWorkspace {
+    char *r, *p, *t, *s, *tmp;
+    double* partial;
+    CgScalars* sc;
+    int nblk;
+};
+
+CgWorkspace carve_cg(const lqcd_ctx* c, void* ws) {
+    CgWorkspace w;
+    const size_t hb = align256(half_bytes(c));
+    char* base = static_cast<char*>(ws);
+    w.r = base; w.p = base + hb; w.t = base + 2 * hb; w.s = base + 3 * hb; w.tmp = base + 4 * hb;
+    w.nblk = (c->g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
+    w.partial = reinterpret_cast<double*>(base + 5 * hb);
+    w.sc = reinterpret_cast<CgScalars*>(base + 5 * hb + align256((size_t)w.nblk * sizeof(double)));
+    return w;
+}
+
+template <typename R>
+lqcd_status cg_loop(const lqcd_ctx* c, void* x, const void* gauge, const void* b, double kappa, double mu, double tol,
+                    int maxiter, const CgWorkspace& w, int* iters_out, double* relres_out, cudaStream_t st) {
+    const size_t hb = half_bytes(c);
+    const double theta = 2.0 * kappa * mu;
+    const Geom& g = c->g;
+    cudaError_t e;
+    lqcd_status s;
+    // x = 0, r = p = b, rr = bb = <b, b>
+    CgScalars init{};
+    init.tol2 = tol * tol;
+    if ((e = cudaMemcpyAsync(w.sc, &init, sizeof(init), cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemsetAsync(x, 0, hb, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(w.r, b, hb, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(w.p, b, hb, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    norm2_kernel<R><<<w.nblk, BLAS_BLOCK, 0, st>>>((const R*)b, g, w.partial);
+    if ((s = after_launch()) != LQCD_OK) return s;
+    cg_scalar_kernel<<<1, BLAS_BLOCK, 0, st>>>(w.partial, w.nblk, w.sc, CG_OP_INIT);
+    if ((s = after_launch()) != LQCD_OK) return s;
+
+    constexpr int CHECK_EVERY = 8;  // iterations enqueued between two looks at the convergence flag
+    CgScalars host{};
+    for (int it = 0; it < maxiter;) {
+        const int chunk = (maxiter - it < CHECK_EVERY) ? maxiter - it : CHECK_EVERY;
+        for (int k = 0; k < chunk; ++k) {
+            // t = Q(mu) p ; alpha = rr / |t|^2
+            if ((s = apply_M_impl(c, w.t, gauge, w.p, kappa, theta, true, 1, w.tmp, st, 1)) != LQCD_OK) return s;
+            norm2_kernel<R><<<w.nblk, BLAS_BLOCK, 0, st>>>((const R*)w.t, g, w.partial);
+            if ((s = after_launch()) != LQCD_OK) return s;
+            cg_scalar_kernel<<<1, BLAS_BLOCK, 0, st>>>(w.partial, w.nblk, w.sc, CG_OP_PAP);
+            if ((s = after_launch()) != LQCD_OK) return s;
+            // s = Q(-mu) t = A p ; x += alpha p ; r -= alpha s ; rr', beta, convergence
+            if ((s = apply_M_impl(c, w.s, gauge, w.t, kappa, -theta, true, 1, w.tmp, st, 1)) != LQCD_OK) return s;
+            cg_update_xr_kernel<R><<<w.nblk, BLAS_BLOCK, 0, st>>>((R*)x, (R*)w.r, (const R*)w.p, (const R*)w.s, g, w.sc, w.partial);
+            if ((s = after_launch()) != LQCD_OK) return s;
+            cg_scalar_kernel<<<1, BLAS_BLOCK, 0, st>>>(w.partial, w.nblk, w.sc, CG_OP_RR);
+            if ((s = after_launch()) != LQCD_OK) return s;
+            cg_update_p_kernel<R><<<w.nblk, BLAS_BLOCK, 0, st>>>((R*)w.p, (const R*)w.r, g, w.sc);
+            if ((s = after_launch()) != LQCD_OK) return s;
+        }
+        it += chunk;
+        if ((e = cudaMemcpyAsync(&host, w.sc, sizeof(host), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+        if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+        if (host.done) break;
+    }
+    if (!host.done) {
+        if ((e = cudaMemcpyAsync(&host, w.sc, sizeof(host), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+        if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+    }
+    if (iters_out) *iters_out = host.iters;
+    if (relres_out) *relres_out = host.bb > 0.0 ? std::sqrt(host.rr / host.bb) : 0.0;
+    return LQCD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t lqcd_cg_workspace_bytes(const lqcd_ctx* c) {
+    if (!c) return 0;
+    const int nblk = (c->g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
+    return 5 * align256(half_bytes(c)) + align256((size_t)nblk * sizeof(double)) + align256(sizeof(CgScalars));
+}
+
+lqcd_status lqcd_apply_Q_tm(const lqcd_ctx* c, void* out, const void* gauge, const void* in, double kappa, double mu,
+                            void* workspace, void* stream) {
+    return apply_M_impl(c, out, gauge, in, kappa, 2.0 * kappa * mu, true, 1, workspace, (cudaStream_t)stream, 1);
+}
+
+lqcd_status lqcd_cg_solve_tm(const lqcd_ctx* c, void* x, const void* gauge, const void* b, double kappa, double mu,
+                             double tol, int maxiter, void* workspace, int* iters_out, double* relres_out, void* stream) {
+    const size_t hb = c ? half_bytes(c) : 0;
+    lqcd_status s = check_fields(c, x, gauge, b, hb);
+    if (s != LQCD_OK) return s;
+    if (!workspace || !(tol > 0.0) || maxiter < 0) return LQCD_EINVAL;
+    if (reinterpret_cast<uintptr_t>(workspace) & 255u) return LQCD_EALIGN;
+    const size_t wb = lqcd_cg_workspace_bytes(c);
+    if (overlaps(workspace, wb, x, hb) || overlaps(workspace, wb, b, hb)) return LQCD_EALIAS;
+    const CgWorkspace w = carve_cg(c, workspace);
+    cudaStream_t st = (cudaStream_t)stream;
+    return c->p.precision == 32 ? cg_loop<float>(c, x, gauge, b, kappa, mu, tol, maxiter, w, iters_out, relres_out, st)
+                                : cg_loop<double>(c, x, gauge, b, kappa, mu, tol, maxiter, w, iters_out, relres_out, st);
 }
 
 lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* c, void* out_host, const void* gauge_host, const void* in_host,
