@@ -333,6 +333,31 @@ def matrix_leg(torch, w, napply=50, reps=3):
     return res
 
 
+def cg_leg(torch, w, mu=0.05, tol=None, maxiter=400):
+    """Next row f2: lqcd_cg_solve_tm on the primary workload (even source = inp[1]).  One iteration = two
+    applications of Q = gamma_5 Mhat_tm (4 dslash launches) + 5 BLAS-1/scalar launches; flops counted by the dslash
+    convention only (4 x 1320 per even site per iteration); bytes: 2 x (2 x (48 + 8 recon) + 24) + 240 reals."""
+    tol = tol or (1e-5 if w.precision == 32 else 1e-10)
+    x = torch.empty_like(w.inp[1])
+    ws = torch.empty(w.ctx.cg_workspace_bytes(), dtype=torch.uint8, device=w.dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    best, it, res = None, 0, 0.0
+    for _ in range(2):
+        torch.cuda.synchronize()
+        e0.record()
+        it, res = w.ctx.cg_solve_tm(x, w.gauge, w.inp[1], w.kappa, mu, tol, maxiter, ws)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None else min(best, ms)
+    enq = -(-it // 8) * 8 if it else 0   # iterations actually enqueued (the flag is checked every 8)
+    reals = 2 * (2 * REALS_PER_SITE[w.recon] + 24) + 240
+    return {"iterations": it, "relres": res, "tol": tol, "kappa": w.kappa, "mu": mu, "ms": best,
+            "us_per_iteration": best * 1e3 / max(enq, 1),
+            "gflops": 4 * FLOP_PER_SITE * w.Vh * enq / (best * 1e-3) / 1e9 if enq else 0.0,
+            "gbs": reals * (w.precision // 8) * w.Vh * enq / (best * 1e-3) / 1e9 if enq else 0.0}
+
+
 def cpu_baseline_leg(cfg_id, precision):
     """The oracle as it stands on the host cores: full-lattice dslash_eo of the same workload,
     one warm-up then best of 3 (about 2-5 s of CPU work on 8+ cores)."""
@@ -423,6 +448,7 @@ def run_b200(args):
 
     if not args.no_extras and rank == 0:
         line["matrix"] = matrix_leg(torch, w)
+        line["cg"] = cg_leg(torch, w)
         line["e2e"] = e2e_leg(torch, w, max(1, min(args.steps, 10)), 1)
     del w
     torch.cuda.empty_cache()
