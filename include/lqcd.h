@@ -146,6 +146,21 @@ lqcd_status lqcd_cg_solve_tm(const lqcd_ctx* ctx, void* x_dev, const void* gauge
                              double mu, double tol, int maxiter, void* workspace_dev, int* iters_out,
                              double* relres_out, void* stream);
 
+/* Mixed-precision CG (fp64 defect correction around the fp32 CG): solves the same equation as lqcd_cg_solve_tm
+ * for fp64 fields to fp64 accuracy while doing the iterations in fp32.
+ *   x = 0, r = b;  repeat { fp32 CG on A e = (float) r to relative tolerance inner_tol;  x += e;  r = b - A x in fp64 }
+ *   until |r| <= tol |b| (r is the TRUE fp64 residual), the total inner iteration count reaches maxiter, or a
+ *   correction brings no progress.
+ * ctx64 / ctx32: contexts of precision 64 / 32 with the same extents and boundary phases (each with its own
+ * recon); gauge64_dev / gauge32_dev: the link field packed for each; x_dev, b_dev: fp64 native even half spinors.
+ * workspace_dev: lqcd_cg_mixed_workspace_bytes bytes, 256-byte aligned.  Synchronises `stream`.
+ * *iters_out = total inner iterations, *outer_out = corrections applied, *relres_out = |b - A x| / |b|. */
+size_t lqcd_cg_mixed_workspace_bytes(const lqcd_ctx* ctx64, const lqcd_ctx* ctx32);
+lqcd_status lqcd_cg_solve_tm_mixed(const lqcd_ctx* ctx64, const lqcd_ctx* ctx32, void* x_dev, const void* gauge64_dev,
+                                   const void* gauge32_dev, const void* b_dev, double kappa, double mu, double tol,
+                                   double inner_tol, int maxiter, void* workspace_dev, int* iters_out, int* outer_out,
+                                   double* relres_out, void* stream);
+
 /* End-to-end convenience for host-resident data: canonical host buffers in, canonical host
  * buffer out.  Copies gauge_host (canonical links; may be NULL to reuse the links packed into
  * workspace_dev by an earlier call) and in_host (canonical half spinor of parity 1-out_parity)

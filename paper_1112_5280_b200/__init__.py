@@ -18,7 +18,7 @@ PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, -1
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
-    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_dslash_eo_host", "lqcd_launch_count",
+    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_launch_count",
     "lqcd_set_block_threads", "lqcd_status_string", "lqcd_last_cuda_error",
 ]
 
@@ -64,6 +64,10 @@ def _lib():
         lib.lqcd_apply_M.argtypes = [vp, vp, vp, vp, cd, ci, vp, vp]
         lib.lqcd_apply_M_tm.argtypes = [vp, vp, vp, vp, cd, cd, ci, vp, vp]
         lib.lqcd_apply_Q_tm.argtypes = [vp, vp, vp, vp, cd, cd, vp, vp]
+        lib.lqcd_cg_mixed_workspace_bytes.argtypes = [vp, vp]
+        lib.lqcd_cg_mixed_workspace_bytes.restype = sz
+        lib.lqcd_cg_solve_tm_mixed.argtypes = [vp, vp, vp, vp, vp, vp, cd, cd, cd, cd, ci, vp, ctypes.POINTER(ci),
+                                               ctypes.POINTER(ci), ctypes.POINTER(cd), vp]
         lib.lqcd_cg_solve_tm.argtypes = [vp, vp, vp, vp, cd, cd, cd, ci, vp, ctypes.POINTER(ci), ctypes.POINTER(cd), vp]
         lib.lqcd_dslash_eo_host.argtypes = [vp, vp, vp, vp, ci, vp, vp]
         lib.lqcd_launch_count.argtypes = []
@@ -169,6 +173,18 @@ class Context:
                                      int(maxiter), _ptr(workspace), ctypes.byref(it), ctypes.byref(res),
                                      _stream(stream)), "lqcd_cg_solve_tm")
         return it.value, res.value
+
+    def cg_mixed_workspace_bytes(self, ctx32):
+        return _lib().lqcd_cg_mixed_workspace_bytes(self._h, ctx32._h)
+
+    def cg_solve_tm_mixed(self, ctx32, x, gauge64, gauge32, b, kappa, mu, tol, inner_tol, maxiter, workspace, stream=None):
+        """self is the fp64 context.  Returns (inner iterations, outer corrections, |b - A x| / |b|)."""
+        it, outer, res = ctypes.c_int(0), ctypes.c_int(0), ctypes.c_double(0.0)
+        _chk(_lib().lqcd_cg_solve_tm_mixed(self._h, ctx32._h, _ptr(x), _ptr(gauge64), _ptr(gauge32), _ptr(b), float(kappa),
+                                           float(mu), float(tol), float(inner_tol), int(maxiter), _ptr(workspace),
+                                           ctypes.byref(it), ctypes.byref(outer), ctypes.byref(res), _stream(stream)),
+             "lqcd_cg_solve_tm_mixed")
+        return it.value, outer.value, res.value
 
     def dslash_eo_host(self, out_host, gauge_host, in_host, out_parity, workspace, stream=None):
         _chk(_lib().lqcd_dslash_eo_host(self._h, _ptr(out_host), _ptr(gauge_host), _ptr(in_host), int(out_parity),

@@ -129,4 +129,59 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_update_p_kernel(R* __restrict__
     store_spinor<R>(p, cb, pv);
 }
 
+// ---- mixed-precision defect correction (fp64 outer, fp32 inner CG) -------------------------------------
+
+// dst = (Rd) src, site by site (the two precisions have different words per site in the native layout)
+template <typename Rd, typename Rs>
+__global__ void __launch_bounds__(BLAS_BLOCK) convert_kernel(Rd* __restrict__ dst, const Rs* __restrict__ src, Geom g) {
+    const int cb = blockIdx.x * BLAS_BLOCK + threadIdx.x;
+    if (cb >= g.Vh) return;
+    Rs a[24];
+    Rd b[24];
+    load_spinor<Rs>(src, cb, a);
+#pragma unroll
+    for (int k = 0; k < 24; ++k) b[k] = (Rd)a[k];
+    store_spinor<Rd>(dst, cb, b);
+}
+
+// x += (double) e
+__global__ void __launch_bounds__(BLAS_BLOCK) accumulate_correction_kernel(double* __restrict__ x, const float* __restrict__ e, Geom g) {
+    const int cb = blockIdx.x * BLAS_BLOCK + threadIdx.x;
+    if (cb >= g.Vh) return;
+    double xv[24];
+    float ev[24];
+    load_spinor<double>(x, cb, xv);
+    load_spinor<float>(e, cb, ev);
+#pragma unroll
+    for (int k = 0; k < 24; ++k) xv[k] += (double)ev[k];
+    store_spinor<double>(x, cb, xv);
+}
+
+// r = b - s;  partial = block sums of |r|^2
+template <typename R>
+__global__ void __launch_bounds__(BLAS_BLOCK) residual_kernel(R* __restrict__ r, const R* __restrict__ b, const R* __restrict__ s,
+                                                               Geom g, double* __restrict__ partial) {
+    const int cb = blockIdx.x * BLAS_BLOCK + threadIdx.x;
+    double n2 = 0.0;
+    if (cb < g.Vh) {
+        R bv[24], sv[24];
+        load_spinor<R>(b, cb, bv);
+        load_spinor<R>(s, cb, sv);
+#pragma unroll
+        for (int k = 0; k < 24; ++k) bv[k] -= sv[k];
+        store_spinor<R>(r, cb, bv);
+        n2 = site_norm2<R>(bv);
+    }
+    n2 = block_sum(n2);
+    if (threadIdx.x == 0) partial[blockIdx.x] = n2;
+}
+
+// One block: *out = sum of partial[0..n) in a fixed order
+__global__ void __launch_bounds__(BLAS_BLOCK) sum_partials_kernel(const double* __restrict__ partial, int n, double* out) {
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n; i += BLAS_BLOCK) s += partial[i];
+    s = block_sum(s);
+    if (threadIdx.x == 0) *out = s;
+}
+
 }  // namespace lqcd

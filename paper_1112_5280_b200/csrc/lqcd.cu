@@ -344,6 +344,21 @@ lqcd_status cg_loop(const lqcd_ctx* c, void* x, const void* gauge, const void* b
     return LQCD_OK;
 }
 
+// |v|^2 of a native half spinor, to host (synchronises the stream)
+template <typename R>
+lqcd_status norm2_to_host(const lqcd_ctx* c, const void* v, double* partial, double* scratch, double* out, cudaStream_t st) {
+    const int nblk = (c->g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
+    lqcd_status s;
+    norm2_kernel<R><<<nblk, BLAS_BLOCK, 0, st>>>((const R*)v, c->g, partial);
+    if ((s = after_launch()) != LQCD_OK) return s;
+    sum_partials_kernel<<<1, BLAS_BLOCK, 0, st>>>(partial, nblk, scratch);
+    if ((s = after_launch()) != LQCD_OK) return s;
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(out, scratch, sizeof(double), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+    return LQCD_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -372,6 +387,89 @@ lqcd_status lqcd_cg_solve_tm(const lqcd_ctx* c, void* x, const void* gauge, cons
     cudaStream_t st = (cudaStream_t)stream;
     return c->p.precision == 32 ? cg_loop<float>(c, x, gauge, b, kappa, mu, tol, maxiter, w, iters_out, relres_out, st)
                                 : cg_loop<double>(c, x, gauge, b, kappa, mu, tol, maxiter, w, iters_out, relres_out, st);
+}
+
+// Mixed precision: fp64 defect correction around the fp32 CG (reading F2).
+//   x = 0, r = b;  repeat { solve A32 e = (float) r to inner_tol with lqcd_cg_solve_tm's loop;  x += e;
+//   r = b - A64 x (true residual, fp64) } until |r| <= tol |b|.
+size_t lqcd_cg_mixed_workspace_bytes(const lqcd_ctx* c64, const lqcd_ctx* c32) {
+    if (!c64 || !c32) return 0;
+    const int nblk = (c64->g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
+    return 4 * align256(half_bytes(c64)) + 2 * align256(half_bytes(c32)) + align256(lqcd_cg_workspace_bytes(c32)) +
+           align256((size_t)nblk * sizeof(double)) + 256;
+}
+
+lqcd_status lqcd_cg_solve_tm_mixed(const lqcd_ctx* c64, const lqcd_ctx* c32, void* x, const void* gauge64,
+                                   const void* gauge32, const void* b, double kappa, double mu, double tol,
+                                   double inner_tol, int maxiter, void* workspace, int* iters_out, int* outer_out,
+                                   double* relres_out, void* stream) {
+    if (!c64 || !c32 || !gauge32) return LQCD_EINVAL;
+    if (c64->p.precision != 64 || c32->p.precision != 32) return LQCD_EINVAL;
+    for (int m = 0; m < 4; ++m)
+        if (c64->p.dims[m] != c32->p.dims[m] || c64->p.bc_re[m] != c32->p.bc_re[m] || c64->p.bc_im[m] != c32->p.bc_im[m])
+            return LQCD_EINVAL;
+    const size_t hb64 = half_bytes(c64), hb32 = half_bytes(c32);
+    lqcd_status s = check_fields(c64, x, gauge64, b, hb64);
+    if (s != LQCD_OK) return s;
+    if (!workspace || !(tol > 0.0) || !(inner_tol > 0.0) || maxiter < 0) return LQCD_EINVAL;
+    if (!aligned16(gauge32)) return LQCD_EALIGN;
+    if (reinterpret_cast<uintptr_t>(workspace) & 255u) return LQCD_EALIGN;
+    const size_t wb = lqcd_cg_mixed_workspace_bytes(c64, c32);
+    if (overlaps(workspace, wb, x, hb64) || overlaps(workspace, wb, b, hb64)) return LQCD_EALIAS;
+
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geom& g = c64->g;
+    const int nblk = (g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
+    char* base = static_cast<char*>(workspace);
+    char* r64 = base;                   base += align256(hb64);
+    char* s64 = base;                   base += align256(hb64);
+    char* t64 = base;                   base += align256(hb64);
+    char* tmp64 = base;                 base += align256(hb64);
+    char* r32 = base;                   base += align256(hb32);
+    char* e32 = base;                   base += align256(hb32);
+    char* inner_ws = base;              base += align256(lqcd_cg_workspace_bytes(c32));
+    double* partial = reinterpret_cast<double*>(base);  base += align256((size_t)nblk * sizeof(double));
+    double* scratch = reinterpret_cast<double*>(base);
+    const CgWorkspace iw = carve_cg(c32, inner_ws);
+    const double theta = 2.0 * kappa * mu;
+
+    cudaError_t e;
+    double bb = 0.0, rr = 0.0;
+    if ((s = norm2_to_host<double>(c64, b, partial, scratch, &bb, st)) != LQCD_OK) return s;
+    if ((e = cudaMemsetAsync(x, 0, hb64, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(r64, b, hb64, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    rr = bb;
+    int total = 0, outer = 0;
+    while (bb > 0.0 && rr > tol * tol * bb && total < maxiter && outer < 50) {
+        // inner solve in fp32: A e = r, relative tolerance inner_tol but never tighter than what is still needed
+        convert_kernel<float, double><<<nblk, BLAS_BLOCK, 0, st>>>((float*)r32, (const double*)r64, g);
+        if ((s = after_launch()) != LQCD_OK) return s;
+        const double need = tol * std::sqrt(bb / rr);  // relative reduction of |r| still required
+        int it = 0;
+        s = cg_loop<float>(c32, e32, gauge32, r32, kappa, mu, inner_tol > 0.5 * need ? inner_tol : 0.5 * need,
+                           maxiter - total, iw, &it, nullptr, st);
+        if (s != LQCD_OK) return s;
+        total += it;
+        ++outer;
+        // x += e;  r = b - A x in fp64
+        accumulate_correction_kernel<<<nblk, BLAS_BLOCK, 0, st>>>((double*)x, (const float*)e32, g);
+        if ((s = after_launch()) != LQCD_OK) return s;
+        if ((s = apply_M_impl(c64, t64, gauge64, x, kappa, theta, true, 1, tmp64, st, 1)) != LQCD_OK) return s;
+        if ((s = apply_M_impl(c64, s64, gauge64, t64, kappa, -theta, true, 1, tmp64, st, 1)) != LQCD_OK) return s;
+        residual_kernel<double><<<nblk, BLAS_BLOCK, 0, st>>>((double*)r64, (const double*)b, (const double*)s64, g, partial);
+        if ((s = after_launch()) != LQCD_OK) return s;
+        sum_partials_kernel<<<1, BLAS_BLOCK, 0, st>>>(partial, nblk, scratch);
+        if ((s = after_launch()) != LQCD_OK) return s;
+        const double rr_old = rr;
+        if ((e = cudaMemcpyAsync(&rr, scratch, sizeof(double), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+        if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+        if (it == 0 || !(rr < rr_old)) break;  // no progress: fp32 cannot reduce this residual further
+    }
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+    if (iters_out) *iters_out = total;
+    if (outer_out) *outer_out = outer;
+    if (relres_out) *relres_out = bb > 0.0 ? std::sqrt(rr / bb) : 0.0;
+    return LQCD_OK;
 }
 
 lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* c, void* out_host, const void* gauge_host, const void* in_host,

@@ -57,3 +57,24 @@ def test_C4_lattice_solution_satisfies_the_equation():
     assert 1 < it < 500 and res <= tol
     assert np.linalg.norm(b - Ax) <= 2 * tol * np.linalg.norm(b)
     assert np.abs(x * (~even)).max() == 0.0
+
+
+def test_C5_mixed_precision_reaches_fp64_accuracy():
+    """Defect correction with an fp32 inner CG: the TRUE fp64 residual (operator composed here) reaches a tolerance
+    far below fp32 epsilon in a few corrections, and the solution is the fp64 CG's."""
+    dims, kappa, mu, tol = (4, 4, 4, 8), 0.15, 0.1, 1e-11
+    U = li.random_su3_links(dims, seed=31)
+    even = li.parity_mask(dims, 0)[..., None, None]
+    b = li.gaussian_spinor(dims, seed=32) * even
+    x, total, outer, res = cg_oracle.cg_mixed_solve_tm(U, b, dims, APBC, kappa, mu, tol, 1e-4, 2000)
+    g5 = np.array([1, 1, -1, -1])[:, None]
+    Ax = g5 * oracle.apply_M_tm(U, g5 * oracle.apply_M_tm(U, x, dims, APBC, kappa, mu, 1), dims, APBC, kappa, -mu, 1)
+    assert np.linalg.norm(b - Ax) <= tol * np.linalg.norm(b) and res <= tol
+    assert 2 <= outer <= 6
+    x64, it64, _ = cg_oracle.cg_solve_tm(U, b, dims, APBC, kappa, mu, tol, 500)
+    assert np.linalg.norm(x - x64) <= 100 * tol * np.linalg.norm(x64)
+    # a single fp32 solve cannot do this: its true residual stalls near fp32 epsilon
+    x32, _, _ = cg_oracle._cg32(lambda v: cg_oracle.normal_operator_tm(U.astype(np.complex64), dims, APBC, kappa, mu)(v).astype(np.complex64),
+                                b.astype(np.complex64), 1e-11, 300)
+    Ax32 = g5 * oracle.apply_M_tm(U, g5 * oracle.apply_M_tm(U, x32.astype(np.complex128), dims, APBC, kappa, mu, 1), dims, APBC, kappa, -mu, 1)
+    assert np.linalg.norm(b - Ax32) > 1e3 * tol * np.linalg.norm(b)
