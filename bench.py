@@ -358,6 +358,25 @@ def cg_leg(torch, w, mu=0.05, tol=None, maxiter=400):
             "gbs": reals * (w.precision // 8) * w.Vh * enq / (best * 1e-3) / 1e9 if enq else 0.0}
 
 
+def cg_mixed_leg(torch, w64, w32, mu=0.05, tol=1e-10, inner_tol=1e-4, maxiter=2000):
+    """lqcd_cg_solve_tm_mixed: the same fp64 system as cg_leg(w64), iterated in fp32 with fp64 defect correction."""
+    b = w64.inp[1]
+    x = torch.empty_like(b)
+    ws = torch.empty(w64.ctx.cg_mixed_workspace_bytes(w32.ctx), dtype=torch.uint8, device=w64.dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    best = None
+    for _ in range(2):
+        torch.cuda.synchronize()
+        e0.record()
+        it, outer, res = w64.ctx.cg_solve_tm_mixed(w32.ctx, x, w64.gauge, w32.gauge, b, w64.kappa, mu, tol, inner_tol, maxiter, ws)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None else min(best, ms)
+    return {"inner_iterations": it, "outer_corrections": outer, "true_relres": res, "tol": tol, "inner_tol": inner_tol,
+            "ms": best}
+
+
 def cpu_baseline_leg(cfg_id, precision):
     """The oracle as it stands on the host cores: full-lattice dslash_eo of the same workload,
     one warm-up then best of 3 (about 2-5 s of CPU work on 8+ cores)."""
@@ -450,8 +469,6 @@ def run_b200(args):
         line["matrix"] = matrix_leg(torch, w)
         line["cg"] = cg_leg(torch, w)
         line["e2e"] = e2e_leg(torch, w, max(1, min(args.steps, 10)), 1)
-    del w
-    torch.cuda.empty_cache()
     if not args.no_extras:
         other = 64 if args.precision == 32 else 32
         w2 = Workload(args.config, other, args.recon, dev, args.block, keep_host=False)
@@ -459,8 +476,14 @@ def run_b200(args):
         line[f"fp{other}"] = {"gflops": r2["gflops"], "achieved_gbs": r2["gbs"], "frac": r2["gbs"] / peak,
                               "frac_of_nominal_8TBs": r2["gbs"] / NOMINAL_HBM_GBS, "us_per_launch": r2["us_per_launch"],
                               "traffic": ncu_traffic(other, args.recon)}
+        if rank == 0:
+            w64, w32 = (w2, w) if other == 64 else (w, w2)
+            line["cg_fp64"] = cg_leg(torch, w64, tol=1e-10)
+            line["cg_mixed"] = cg_mixed_leg(torch, w64, w32, tol=1e-10)
         del w2
-        torch.cuda.empty_cache()
+    del w
+    torch.cuda.empty_cache()
+    if not args.no_extras:
         if rank == 0:
             if args.chain:  # config 5; opt-in: generating its 3 GB A11 link field takes minutes of host time
                 import numpy as np
