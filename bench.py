@@ -53,6 +53,7 @@ def parse_args():
     ap.add_argument("--block", type=int, default=0, help="dslash block size override (tuning)")
     ap.add_argument("--chain", action="store_true", help="also time config 5: apply_M(eo=1) x100 chained at 48^3x96")
     ap.add_argument("--no-extras", action="store_true", help="skip the fp64 / chain / e2e / cpu legs (profiling runs)")
+    ap.add_argument("--legs", default="all", help="comma list of extra legs to run: matrix,cg,e2e,other,cgmixed,cpu (default all)")
     return ap.parse_args()
 
 
@@ -234,8 +235,9 @@ def kernel_leg(torch, dist, w, steps, warmup, world):
 
 
 def e2e_leg(torch, w, steps, world):
-    """Same metric through the host-buffer entry point lqcd_dslash_eo_host: pinned canonical half
-    spinor in (H2D), pack, dslash, unpack, canonical half spinor out (D2H) inside the timed region.
+    """Same metric through the host-buffer entry point lqcd_dslash_eo_host_batch: per item pinned canonical half
+    spinor in (H2D), pack, dslash, unpack, canonical half spinor out (D2H), all inside the timed region; the
+    library overlaps upload, kernels and download of consecutive items on three streams.
     The link field is uploaded once before (it is constant across applications, like weights)."""
     ctx = w.ctx
     ws = torch.empty(ctx.host_workspace_bytes(), dtype=torch.uint8, device=w.dev)
@@ -250,14 +252,13 @@ def e2e_leg(torch, w, steps, world):
         e1.record()
         torch.cuda.synchronize()
         tg.append(e0.elapsed_time(e1))
-    for b in range(w.nbuf):  # warm-up
-        ctx.dslash_eo_host(out_h[b], None, w.in_host[b], b & 1, ws)
+    par = [b & 1 for b in range(w.nbuf)]
+    ctx.dslash_eo_host_batch(out_h, None, w.in_host, par, ws)  # warm-up
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     e0.record()
     for _ in range(steps):
-        for b in range(w.nbuf):
-            ctx.dslash_eo_host(out_h[b], None, w.in_host[b], b & 1, ws)
+        ctx.dslash_eo_host_batch(out_h, None, w.in_host, par, ws)  # one step = the batch of NBUF half spinors
     e1.record()
     torch.cuda.synchronize()
     wall = (time.perf_counter() - t0) * 1e3
@@ -465,25 +466,30 @@ def run_b200(args):
         },
     }
 
-    if not args.no_extras and rank == 0:
-        line["matrix"] = matrix_leg(torch, w)
-        line["cg"] = cg_leg(torch, w)
-        line["e2e"] = e2e_leg(torch, w, max(1, min(args.steps, 10)), 1)
-    if not args.no_extras:
+    legs = set() if args.no_extras else set(args.legs.split(","))
+    want = lambda name: "all" in legs or name in legs
+    if rank == 0:
+        if want("matrix"):
+            line["matrix"] = matrix_leg(torch, w)
+        if want("cg"):
+            line["cg"] = cg_leg(torch, w)
+        if want("e2e"):
+            line["e2e"] = e2e_leg(torch, w, max(1, min(args.steps, 10)), 1)
+    if want("other"):
         other = 64 if args.precision == 32 else 32
         w2 = Workload(args.config, other, args.recon, dev, args.block, keep_host=False)
         r2 = kernel_leg(torch, dist, w2, max(1, args.steps // 2), args.warmup, world)
         line[f"fp{other}"] = {"gflops": r2["gflops"], "achieved_gbs": r2["gbs"], "frac": r2["gbs"] / peak,
                               "frac_of_nominal_8TBs": r2["gbs"] / NOMINAL_HBM_GBS, "us_per_launch": r2["us_per_launch"],
                               "traffic": ncu_traffic(other, args.recon)}
-        if rank == 0:
+        if rank == 0 and want("cgmixed"):
             w64, w32 = (w2, w) if other == 64 else (w, w2)
             line["cg_fp64"] = cg_leg(torch, w64, tol=1e-10)
             line["cg_mixed"] = cg_mixed_leg(torch, w64, w32, tol=1e-10)
         del w2
     del w
     torch.cuda.empty_cache()
-    if not args.no_extras:
+    if want("cpu") or args.chain:
         if rank == 0:
             if args.chain:  # config 5; opt-in: generating its 3 GB A11 link field takes minutes of host time
                 import numpy as np
@@ -491,7 +497,8 @@ def run_b200(args):
                 U5 = li.links_for_config(5, dtype=np.complex64)
                 line["chain"] = [chain_leg(torch, 5, 32, rc, dev, U=U5) for rc in (12, 18)]
                 del U5
-            line["cpu_baseline"] = cpu_baseline_leg(args.config, args.precision)
+            if want("cpu"):
+                line["cpu_baseline"] = cpu_baseline_leg(args.config, args.precision)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()

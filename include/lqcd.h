@@ -161,13 +161,18 @@ lqcd_status lqcd_cg_solve_tm_mixed(const lqcd_ctx* ctx64, const lqcd_ctx* ctx32,
                                    double inner_tol, int maxiter, void* workspace_dev, int* iters_out, int* outer_out,
                                    double* relres_out, void* stream);
 
-/* End-to-end convenience for host-resident data: canonical host buffers in, canonical host
- * buffer out.  Copies gauge_host (canonical links; may be NULL to reuse the links packed into
- * workspace_dev by an earlier call) and in_host (canonical half spinor of parity 1-out_parity)
- * to the device, packs, runs lqcd_dslash_eo, unpacks, copies the canonical half spinor of
- * parity out_parity to out_host and synchronises `stream`.  workspace_dev is device scratch
- * of lqcd_host_workspace_bytes bytes, 256-byte aligned, owned by the caller.  Host buffers
- * should be pinned for full PCIe speed (pageable memory works, slower). */
+/* End-to-end path for host-resident data: canonical host buffers in, canonical host buffers out.
+ * For each of the n items: copy in_host[i] (canonical half spinor of parity 1 - out_parity[i]) to the device,
+ * pack, lqcd_dslash_eo, unpack, copy the canonical half spinor of parity out_parity[i] to out_host[i].
+ * Items are pipelined over three device slots and three streams (upload / kernels on `stream` / download), so
+ * both PCIe directions and the kernels overlap.  gauge_host: canonical links, uploaded and packed first; NULL
+ * reuses the links packed into workspace_dev by an earlier call.  workspace_dev: device scratch of
+ * lqcd_host_workspace_bytes bytes, 256-byte aligned, owned by the caller.  Host buffers should be pinned
+ * (pageable memory works, without overlap).  Work already enqueued on `stream` is ordered before the call; the
+ * call synchronises before returning (its results live in host memory).  lqcd_dslash_eo_host is the n = 1 case. */
+lqcd_status lqcd_dslash_eo_host_batch(const lqcd_ctx* ctx, int n, void* const* out_host, const void* gauge_host,
+                                      const void* const* in_host, const int* out_parity, void* workspace_dev,
+                                      void* stream);
 lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* ctx, void* out_host, const void* gauge_host,
                                 const void* in_host, int out_parity, void* workspace_dev, void* stream);
 

@@ -18,7 +18,7 @@ PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, -1
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
-    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_launch_count",
+    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_dslash_eo_host_batch", "lqcd_launch_count",
     "lqcd_set_block_threads", "lqcd_status_string", "lqcd_last_cuda_error",
 ]
 
@@ -70,6 +70,7 @@ def _lib():
                                                ctypes.POINTER(ci), ctypes.POINTER(cd), vp]
         lib.lqcd_cg_solve_tm.argtypes = [vp, vp, vp, vp, cd, cd, cd, ci, vp, ctypes.POINTER(ci), ctypes.POINTER(cd), vp]
         lib.lqcd_dslash_eo_host.argtypes = [vp, vp, vp, vp, ci, vp, vp]
+        lib.lqcd_dslash_eo_host_batch.argtypes = [vp, ci, ctypes.POINTER(vp), vp, ctypes.POINTER(vp), ctypes.POINTER(ci), vp, vp]
         lib.lqcd_launch_count.argtypes = []
         lib.lqcd_launch_count.restype = ctypes.c_ulonglong
         lib.lqcd_set_block_threads.argtypes = [vp, ci]
@@ -189,6 +190,15 @@ class Context:
     def dslash_eo_host(self, out_host, gauge_host, in_host, out_parity, workspace, stream=None):
         _chk(_lib().lqcd_dslash_eo_host(self._h, _ptr(out_host), _ptr(gauge_host), _ptr(in_host), int(out_parity),
                                         _ptr(workspace), _stream(stream)), "lqcd_dslash_eo_host")
+
+    def dslash_eo_host_batch(self, outs_host, gauge_host, ins_host, out_parities, workspace, stream=None):
+        n = len(outs_host)
+        assert len(ins_host) == n and len(out_parities) == n
+        outs = (ctypes.c_void_p * n)(*[_ptr(t) for t in outs_host])
+        ins = (ctypes.c_void_p * n)(*[_ptr(t) for t in ins_host])
+        par = (ctypes.c_int * n)(*[int(p) for p in out_parities])
+        _chk(_lib().lqcd_dslash_eo_host_batch(self._h, n, outs, _ptr(gauge_host), ins, par, _ptr(workspace),
+                                              _stream(stream)), "lqcd_dslash_eo_host_batch")
 
 
 def launch_count() -> int:

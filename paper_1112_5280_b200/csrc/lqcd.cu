@@ -48,6 +48,7 @@ inline bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
 inline size_t elem(const lqcd_ctx* c) { return c->p.precision == 32 ? 4 : 8; }
 inline size_t half_bytes(const lqcd_ctx* c) { return (size_t)24 * TILE * c->g.ntiles * elem(c); }  // padded to whole tiles
 inline size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
+constexpr int HOST_SLOTS = 3;  // pipeline depth of lqcd_dslash_eo_host_batch
 
 template <typename R>
 BcPhases<R> make_bc(const lqcd_ctx* c) {
@@ -167,7 +168,7 @@ size_t lqcd_workspace_bytes(const lqcd_ctx* c) { return c ? half_bytes(c) : 0; }
 size_t lqcd_host_workspace_bytes(const lqcd_ctx* c) {
     if (!c) return 0;
     const size_t canon_gauge = (size_t)4 * 2 * c->g.Vh * 18 * elem(c);
-    return align256(lqcd_gauge_bytes(c)) + align256(canon_gauge) + 4 * align256(half_bytes(c));
+    return align256(lqcd_gauge_bytes(c)) + align256(canon_gauge) + HOST_SLOTS * 4 * align256(half_bytes(c));
 }
 
 lqcd_status lqcd_set_block_threads(lqcd_ctx* c, int b) {
@@ -472,34 +473,91 @@ lqcd_status lqcd_cg_solve_tm_mixed(const lqcd_ctx* c64, const lqcd_ctx* c32, voi
     return LQCD_OK;
 }
 
-lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* c, void* out_host, const void* gauge_host, const void* in_host,
-                                int out_parity, void* ws, void* stream) {
-    if (!c || !out_host || !in_host || !ws) return LQCD_EINVAL;
-    if (out_parity != 0 && out_parity != 1) return LQCD_EINVAL;
+// Host-buffer path.  Items are pipelined over HOST_SLOTS device slots and three streams (upload, the caller's
+// stream for the kernels, download), so the two PCIe directions and the kernels overlap.
+lqcd_status lqcd_dslash_eo_host_batch(const lqcd_ctx* c, int n, void* const* out_host, const void* gauge_host,
+                                      const void* const* in_host, const int* out_parity, void* ws, void* stream) {
+    if (!c || n < 0 || (n > 0 && (!out_host || !in_host || !out_parity)) || !ws) return LQCD_EINVAL;
+    for (int i = 0; i < n; ++i)
+        if (!out_host[i] || !in_host[i] || (out_parity[i] != 0 && out_parity[i] != 1)) return LQCD_EINVAL;
     if (reinterpret_cast<uintptr_t>(ws) & 255u) return LQCD_EALIGN;
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t hb = half_bytes(c);
+    const size_t hb = half_bytes(c);                             // native half spinor (padded to whole tiles)
+    const size_t cb_bytes = (size_t)24 * c->g.Vh * elem(c);     // canonical half spinor
     const size_t canon_gauge = (size_t)4 * 2 * c->g.Vh * 18 * elem(c);
     char* base = static_cast<char*>(ws);
     char* g_nat = base;                 base += align256(lqcd_gauge_bytes(c));
     char* g_can = base;                 base += align256(canon_gauge);
-    char* in_can = base;                base += align256(hb);
-    char* in_nat = base;                base += align256(hb);
-    char* out_nat = base;               base += align256(hb);
-    char* out_can = base;
-    cudaError_t e;
-    lqcd_status s;
-    if (gauge_host) {
-        if ((e = cudaMemcpyAsync(g_can, gauge_host, canon_gauge, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
-        if ((s = lqcd_pack_gauge(c, g_nat, g_can, stream)) != LQCD_OK) return s;
+    char *in_can[HOST_SLOTS], *in_nat[HOST_SLOTS], *out_nat[HOST_SLOTS], *out_can[HOST_SLOTS];
+    for (int k = 0; k < HOST_SLOTS; ++k) {
+        in_can[k] = base;  base += align256(hb);
+        in_nat[k] = base;  base += align256(hb);
+        out_nat[k] = base; base += align256(hb);
+        out_can[k] = base; base += align256(hb);
     }
-    if ((e = cudaMemcpyAsync(in_can, in_host, hb, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
-    if ((s = lqcd_pack_spinor(c, in_nat, in_can, 1 - out_parity, stream)) != LQCD_OK) return s;
-    if ((s = lqcd_dslash_eo(c, out_nat, g_nat, in_nat, out_parity, stream)) != LQCD_OK) return s;
-    if ((s = lqcd_unpack_spinor(c, out_can, out_nat, out_parity, stream)) != LQCD_OK) return s;
-    if ((e = cudaMemcpyAsync(out_host, out_can, hb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
-    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
-    return LQCD_OK;
+    cudaError_t e = cudaSuccess;
+    lqcd_status s = LQCD_OK;
+    cudaStream_t up = nullptr, down = nullptr;
+    cudaEvent_t start = nullptr, in_done[HOST_SLOTS] = {}, comp_done[HOST_SLOTS] = {}, out_done[HOST_SLOTS] = {};
+    auto fail = [&](cudaError_t err) { e = err; return err != cudaSuccess; };
+    do {
+        if (fail(cudaStreamCreateWithFlags(&up, cudaStreamNonBlocking))) break;
+        if (fail(cudaStreamCreateWithFlags(&down, cudaStreamNonBlocking))) break;
+        if (fail(cudaEventCreateWithFlags(&start, cudaEventDisableTiming))) break;
+        bool ok = true;
+        for (int k = 0; k < HOST_SLOTS && ok; ++k)
+            ok = !fail(cudaEventCreateWithFlags(&in_done[k], cudaEventDisableTiming)) &&
+                 !fail(cudaEventCreateWithFlags(&comp_done[k], cudaEventDisableTiming)) &&
+                 !fail(cudaEventCreateWithFlags(&out_done[k], cudaEventDisableTiming));
+        if (!ok) break;
+        // everything already enqueued on the caller's stream comes first
+        if (fail(cudaEventRecord(start, st)) || fail(cudaStreamWaitEvent(up, start, 0)) || fail(cudaStreamWaitEvent(down, start, 0))) break;
+        if (gauge_host) {
+            if (fail(cudaMemcpyAsync(g_can, gauge_host, canon_gauge, cudaMemcpyHostToDevice, st))) break;
+            if ((s = lqcd_pack_gauge(c, g_nat, g_can, stream)) != LQCD_OK) break;
+        }
+        for (int i = 0; i < n; ++i) {
+            const int k = i % HOST_SLOTS;
+            // upload: the slot's previous kernels must have consumed in_can
+            if (i >= HOST_SLOTS && fail(cudaStreamWaitEvent(up, comp_done[k], 0))) break;
+            if (fail(cudaMemcpyAsync(in_can[k], in_host[i], cb_bytes, cudaMemcpyHostToDevice, up))) break;
+            if (fail(cudaEventRecord(in_done[k], up))) break;
+            // kernels on the caller's stream: the slot's previous download must have drained out_can
+            if (fail(cudaStreamWaitEvent(st, in_done[k], 0))) break;
+            if (i >= HOST_SLOTS && fail(cudaStreamWaitEvent(st, out_done[k], 0))) break;
+            if ((s = lqcd_pack_spinor(c, in_nat[k], in_can[k], 1 - out_parity[i], stream)) != LQCD_OK) break;
+            if ((s = lqcd_dslash_eo(c, out_nat[k], g_nat, in_nat[k], out_parity[i], stream)) != LQCD_OK) break;
+            if ((s = lqcd_unpack_spinor(c, out_can[k], out_nat[k], out_parity[i], stream)) != LQCD_OK) break;
+            if (fail(cudaEventRecord(comp_done[k], st))) break;
+            // download
+            if (fail(cudaStreamWaitEvent(down, comp_done[k], 0))) break;
+            if (fail(cudaMemcpyAsync(out_host[i], out_can[k], cb_bytes, cudaMemcpyDeviceToHost, down))) break;
+            if (fail(cudaEventRecord(out_done[k], down))) break;
+        }
+    } while (false);
+    // drain all three streams before the events and streams go away (also on the error paths)
+    if (up) cudaStreamSynchronize(up);
+    if (down) cudaStreamSynchronize(down);
+    const cudaError_t es = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = es;
+    for (int k = 0; k < HOST_SLOTS; ++k) {
+        if (in_done[k]) cudaEventDestroy(in_done[k]);
+        if (comp_done[k]) cudaEventDestroy(comp_done[k]);
+        if (out_done[k]) cudaEventDestroy(out_done[k]);
+    }
+    if (start) cudaEventDestroy(start);
+    if (up) cudaStreamDestroy(up);
+    if (down) cudaStreamDestroy(down);
+    if (s != LQCD_OK) return s;
+    return e == cudaSuccess ? LQCD_OK : cuda_fail(e);
+}
+
+lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* c, void* out_host, const void* gauge_host, const void* in_host,
+                                int out_parity, void* ws, void* stream) {
+    if (!out_host || !in_host) return LQCD_EINVAL;
+    void* outs[1] = {out_host};
+    const void* ins[1] = {in_host};
+    return lqcd_dslash_eo_host_batch(c, 1, outs, gauge_host, ins, &out_parity, ws, stream);
 }
 
 unsigned long long lqcd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
