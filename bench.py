@@ -351,7 +351,7 @@ def cg_leg(torch, w, mu=0.05, tol=None, maxiter=400):
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1)
         best = ms if best is None else min(best, ms)
-    enq = -(-it // 8) * 8 if it else 0   # iterations actually enqueued (the flag is checked every 8)
+    enq = it   # the flag is read every iteration near convergence, so (almost) no iteration is enqueued in vain
     reals = 2 * (2 * REALS_PER_SITE[w.recon] + 24) + 240
     return {"iterations": it, "relres": res, "tol": tol, "kappa": w.kappa, "mu": mu, "ms": best,
             "us_per_iteration": best * 1e3 / max(enq, 1),
@@ -396,8 +396,14 @@ def cpu_baseline_leg(cfg_id, precision):
         oracle.dslash_eo(U, psi, c["dims"], c["bc"], 0)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
-    return {"value": Vh * FLOP_PER_SITE / best / 1e9, "unit": "GFLOP/s", "cores": oracle.num_threads(),
-            "kind": "oracle",
+    nthreads = oracle.num_threads()
+    oracle.set_num_threads(1)
+    t0 = time.perf_counter()
+    oracle.dslash_eo(U, psi, c["dims"], c["bc"], 0)
+    one = time.perf_counter() - t0
+    oracle.set_num_threads(nthreads)
+    return {"value": Vh * FLOP_PER_SITE / best / 1e9, "unit": "GFLOP/s", "cores": nthreads,
+            "value_1_thread": Vh * FLOP_PER_SITE / one / 1e9, "kind": "oracle",
             "sample": f"config {cfg_id}: one full oracle.dslash_eo (V/2 = {Vh} output sites, fp64 arithmetic on "
                       f"fp{precision} inputs), best of 3 after one warm-up, {best * 1e3:.0f} ms"}
 
@@ -455,6 +461,9 @@ def run_b200(args):
         },
         "gpu_launches": main["launches"],
         "achieved_gbs": main["gbs"],
+        # community "no-reuse" convention (8 neighbour spinors + output + 8 links per site: counts L2 hits; the
+        # paper's 105 GB/s on an AMD 5870, is by inference quoted this way with 18-real links)
+        "effective_gbs_no_reuse": main["gbs"] * (8 * 24 + 24 + 8 * args.recon) / REALS_PER_SITE[args.recon],
         "us_per_launch": main["us_per_launch"],
         "clocks": clocks,
         "roofline": {

@@ -138,7 +138,8 @@ lqcd_status lqcd_apply_Q_tm(const lqcd_ctx* ctx, void* out_dev, const void* gaug
  * x_dev, b_dev: native even half spinors (b is not modified; x must not overlap b).  workspace_dev:
  * lqcd_cg_workspace_bytes(ctx) bytes of device scratch, 256-byte aligned.  All vector updates, reductions and
  * scalars (alpha, beta, <r,r>, the convergence flag) stay on the device; the host looks at the flag every 8
- * iterations, and iterations enqueued after convergence leave x untouched.  Reductions are deterministic.
+ * iterations (every iteration once |r|^2 is within 1000x of the target), and iterations enqueued after convergence
+ * leave x untouched.  Reductions are deterministic.
  * The call synchronises `stream` before returning: *iters_out = iterations performed, *relres_out = |r| / |b|
  * of the recursive residual (host pointers, either may be NULL).  Arithmetic in the ctx precision. */
 size_t lqcd_cg_workspace_bytes(const lqcd_ctx* ctx);

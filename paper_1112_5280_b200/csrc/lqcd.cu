@@ -311,10 +311,14 @@ lqcd_status cg_loop(const lqcd_ctx* c, void* x, const void* gauge, const void* b
     cg_scalar_kernel<<<1, BLAS_BLOCK, 0, st>>>(w.partial, w.nblk, w.sc, CG_OP_INIT);
     if ((s = after_launch()) != LQCD_OK) return s;
 
-    constexpr int CHECK_EVERY = 8;  // iterations enqueued between two looks at the convergence flag
+    // Iterations enqueued between two looks at the convergence flag: 8 while the residual is far from the
+    // target, 1 once |r|^2 is within a factor 1000 of it (so at most a few iterations are enqueued in vain).
+    constexpr int CHECK_EVERY = 8;
     CgScalars host{};
+    host.rr = host.bb = 1.0;
     for (int it = 0; it < maxiter;) {
-        const int chunk = (maxiter - it < CHECK_EVERY) ? maxiter - it : CHECK_EVERY;
+        const int want = host.rr <= 1e3 * init.tol2 * host.bb ? 1 : CHECK_EVERY;
+        const int chunk = (maxiter - it < want) ? maxiter - it : want;
         for (int k = 0; k < chunk; ++k) {
             // t = Q(mu) p ; alpha = rr / |t|^2
             if ((s = apply_M_impl(c, w.t, gauge, w.p, kappa, theta, true, 1, w.tmp, st, 1)) != LQCD_OK) return s;
