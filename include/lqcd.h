@@ -39,6 +39,9 @@
  *     first `recon` reals of 18).  W = 16 bytes / sizeof(element) reals per 128-bit word.
  *     half spinor  word q = r / W, lane = r % W  at element ((cb/32 * 24/W + q) * 32 + cb%32) * W + lane
  *     full spinor  [even half | odd half], each of lqcd_spinor_bytes(ctx, 1) bytes
+ *     precision 16: a half spinor is 3 16-byte words of 8 halfs per site, [tile][word 3][32], holding v / n(x),
+ *                  n(x) = max |component|, followed by the fp32 norms n(x), float[32 ntiles]; links are 3 8-byte words
+ *                  of 4 halfs, [parity][tile][hop 8][word 3][32] (52 bytes per spinor site, 24 per link)
  *     links        gathered by output site: [parity p of x][tile][hop k 8][word][32][lane], hop k = 2 mu holds
  *                  U_mu(x), k = 2 mu + 1 holds U_mu(x - mu^) (stored as is; the kernel takes the adjoint).
  *                  Words of 4 floats (recon 12, 3 words), 2 floats (precision 32 recon 18, 9 words of
@@ -68,7 +71,9 @@ typedef enum {
 
 typedef struct {
     int dims[4];      /* X,Y,Z,T (mu = 0..3); each even and >= 4 (reading A17) */
-    int precision;    /* 32 or 64: storage and arithmetic type of all fields */
+    int precision;    /* 64 or 32: storage and arithmetic type of all fields; 16: fields stored as IEEE half
+                         (spinors normalised per site, with an fp32 norm), fp32 arithmetic, recon 12 only;
+                         canonical buffers are complex64; the CG entry points return LQCD_EUNSUPPORTED */
     int recon;        /* 18 or 12: stored reals per link; 12 = two rows, third rebuilt in
                          registers as conj(row0 x row1) ("RECONSTRUCT TWELVE") */
     double bc_re[4];  /* boundary phase bc_mu = bc_re + i bc_im, |bc_mu| = 1 within 1e-12; */

@@ -206,10 +206,11 @@ def launch_count() -> int:
 
 
 def real_dtype(precision):
+    """dtype of the canonical (interchange) buffers: precision 16 exchanges complex64 like precision 32."""
     import torch
-    return torch.float32 if precision == 32 else torch.float64
+    return torch.float64 if precision == 64 else torch.float32
 
 
 def complex_dtype(precision):
     import torch
-    return torch.complex64 if precision == 32 else torch.complex128
+    return torch.complex128 if precision == 64 else torch.complex64

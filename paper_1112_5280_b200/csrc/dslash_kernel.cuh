@@ -53,7 +53,8 @@ template <typename R> struct BcPhases { R re[4], im[4]; };
 // The arithmetic of one of the eight hops on a gathered neighbour spinor v and link u:
 // project (K3), boundary phase (K3b), colour multiply (K4), reconstruct + accumulate (K5).
 template <typename R, bool CBC, int MU, bool FWD>
-__device__ __forceinline__ void hop_math(R acc[24], const R v[24], const R u[18], bool cross, const BcPhases<R>& bc) {
+__device__ __forceinline__ void hop_math(R acc[24], const R v[24], R scale, const R u[18], bool cross,
+                                         const BcPhases<R>& bc) {
     constexpr int S = FWD ? +1 : -1;
     using P = Proj<MU>;
 
@@ -71,7 +72,9 @@ __device__ __forceinline__ void hop_math(R acc[24], const R v[24], const R u[18]
 
     // K3b: psi(x + L mu^) = bc psi(x): forward crossing multiplies by bc_mu, backward by conj(bc_mu).
     // Real (+-1) phases cost nothing: the sign f rides on the accumulation FMAs of K5.
-    R f = R(1);
+    // the neighbour spinor is scale * v (16-bit storage keeps a norm per site; scale = 1 otherwise): the hop is
+    // linear, so the scale rides on f too
+    R f = scale;
     if (CBC) {
         if (cross) {
             const R br = bc.re[MU], bi = FWD ? bc.im[MU] : -bc.im[MU];
@@ -83,7 +86,7 @@ __device__ __forceinline__ void hop_math(R acc[24], const R v[24], const R u[18]
             }
         }
     } else {
-        f = cross ? bc.re[MU] : R(1);
+        f = cross ? bc.re[MU] * scale : scale;
     }
 
     // K4: chi = U h (forward) or U^+ h (backward), both spin components; explicit FMA chains
@@ -126,17 +129,19 @@ __device__ __forceinline__ void hop_math(R acc[24], const R v[24], const R u[18]
 }
 
 // Hop K = 2 mu + (backward ? 1 : 0): gather the neighbour spinor and the link stored for this hop
-// (U_mu(x) or U_mu(x - mu^), fields.cuh), then the arithmetic.
-template <typename R, int RECON, bool CBC, int K>
-__device__ __forceinline__ void hop_step(R acc[24], const typename LinkWord<R, RECON>::type* __restrict__ site_links,
-                                         const R* __restrict__ in, const int nb[8], unsigned crossmask,
-                                         const BcPhases<R>& bc) {
+// (U_mu(x) or U_mu(x - mu^), fields.cuh), then the arithmetic.  S = storage type, R = arithmetic type.
+template <typename S, int RECON, bool CBC, int K>
+__device__ __forceinline__ void hop_step(typename Compute<S>::type acc[24],
+                                         const typename LinkStore<S, RECON>::word* __restrict__ site_links,
+                                         const S* __restrict__ in, int ntiles, const int nb[8], unsigned crossmask,
+                                         const BcPhases<typename Compute<S>::type>& bc) {
+    using R = typename Compute<S>::type;
     constexpr int MU = K / 2;
     constexpr bool FWD = (K & 1) == 0;
-    R v[24], u[18];
-    load_spinor<R>(in, nb[K], v);
-    load_link<R, RECON>(site_links, K, u);
-    hop_math<R, CBC, MU, FWD>(acc, v, u, (crossmask >> K) & 1u, bc);
+    R v[24], u[18], scale;
+    load_field<S>(in, ntiles, nb[K], v, scale);
+    if constexpr (sizeof(S) == 2) load_link_h(site_links, K, u); else load_link<R, RECON>(site_links, K, u);
+    hop_math<R, CBC, MU, FWD>(acc, v, scale, u, (crossmask >> K) & 1u, bc);
 }
 
 // Resident 64-thread blocks per SM promised to ptxas (__launch_bounds__ min blocks).  The hint sets the
@@ -155,11 +160,15 @@ __device__ __forceinline__ void hop_step(R acc[24], const typename LinkWord<R, R
 #ifndef LQCD_MINB_F64_R18
 #define LQCD_MINB_F64_R18 4
 #endif
+#ifndef LQCD_MINB_F16_R12
+#define LQCD_MINB_F16_R12 8
+#endif
 template <typename R, int RECON> struct MinBlocks;
 template <> struct MinBlocks<float, 12>  { static constexpr int value = LQCD_MINB_F32_R12; };
 template <> struct MinBlocks<float, 18>  { static constexpr int value = LQCD_MINB_F32_R18; };
 template <> struct MinBlocks<double, 12> { static constexpr int value = LQCD_MINB_F64_R12; };
 template <> struct MinBlocks<double, 18> { static constexpr int value = LQCD_MINB_F64_R18; };
+template <> struct MinBlocks<__half, 12>  { static constexpr int value = LQCD_MINB_F16_R12; };
 
 // Step K6, the epilogue applied to acc = (H in)(x) before the store (EPI):
 //   EPI_STORE    out = acc                                        lqcd_dslash_*
@@ -186,15 +195,17 @@ __device__ __forceinline__ void g5_scale(R v[24], R g_re, R g_im) {
 
 // grid.y = 1: one parity `parity0`; grid.y = 2: both, parity = blockIdx.y, and in/out/xin are
 // full fields [even|odd] (in is read at the opposite half).  One thread per output site.
-template <typename R, int RECON, int EPI, bool CBC, int BLOCK>
-__global__ void __launch_bounds__(BLOCK, MinBlocks<R, RECON>::value * 64 / BLOCK)
-dslash_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __restrict__ in,
-              const R* __restrict__ xin, Epilogue<R> epi, Geom g, int parity0, BcPhases<R> bc) {
+// S = storage type of all fields (float, double, or __half with fp32 arithmetic), R = arithmetic type.
+template <typename S, int RECON, int EPI, bool CBC, int BLOCK>
+__global__ void __launch_bounds__(BLOCK, MinBlocks<S, RECON>::value * 64 / BLOCK)
+dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restrict__ in, const S* __restrict__ xin,
+              Epilogue<typename Compute<S>::type> epi, Geom g, int parity0, BcPhases<typename Compute<S>::type> bc) {
+    using R = typename Compute<S>::type;
     constexpr bool XPAY = EPI == EPI_XPAY || EPI == EPI_G5XPAY;
     int p = parity0;
     if (gridDim.y == 2) {
         p = blockIdx.y;
-        const size_t half = (size_t)24 * TILE * g.ntiles;
+        const size_t half = half_stride<S>(g.ntiles);
         in += (size_t)(1 - p) * half;
         out += (size_t)p * half;
         if (XPAY) xin += (size_t)p * half;
@@ -217,26 +228,30 @@ dslash_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __restr
         nb[6] = neighbour<3, true>(g, cb, s, c);  crossmask |= (unsigned)c << 6;
         nb[7] = neighbour<3, false>(g, cb, s, c); crossmask |= (unsigned)c << 7;
     }
-    const auto* site_links =
-        reinterpret_cast<const typename LinkWord<R, RECON>::type*>(gauge) + link_word0<R, RECON>(g.ntiles, p, cb, 0);
+    const auto* site_links = reinterpret_cast<const typename LinkStore<S, RECON>::word*>(gauge) +
+                             LinkStore<S, RECON>::word0(g.ntiles, p, cb, 0);
 
     R acc[24];
 #pragma unroll
     for (int k = 0; k < 24; ++k) acc[k] = 0;
 
-    hop_step<R, RECON, CBC, 0>(acc, site_links, in, nb, crossmask, bc);
-    hop_step<R, RECON, CBC, 1>(acc, site_links, in, nb, crossmask, bc);
-    hop_step<R, RECON, CBC, 2>(acc, site_links, in, nb, crossmask, bc);
-    hop_step<R, RECON, CBC, 3>(acc, site_links, in, nb, crossmask, bc);
-    hop_step<R, RECON, CBC, 4>(acc, site_links, in, nb, crossmask, bc);
-    hop_step<R, RECON, CBC, 5>(acc, site_links, in, nb, crossmask, bc);
-    hop_step<R, RECON, CBC, 6>(acc, site_links, in, nb, crossmask, bc);
-    hop_step<R, RECON, CBC, 7>(acc, site_links, in, nb, crossmask, bc);
+    hop_step<S, RECON, CBC, 0>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
+    hop_step<S, RECON, CBC, 1>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
+    hop_step<S, RECON, CBC, 2>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
+    hop_step<S, RECON, CBC, 3>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
+    hop_step<S, RECON, CBC, 4>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
+    hop_step<S, RECON, CBC, 5>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
+    hop_step<S, RECON, CBC, 6>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
+    hop_step<S, RECON, CBC, 7>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
 
     if constexpr (EPI == EPI_G5SCALE) g5_scale<R>(acc, epi.g_re, epi.g_im);
     if constexpr (XPAY) {
-        R x[24];
-        load_spinor<R>(xin, cb, x);
+        R x[24], xs;
+        load_field<S>(xin, g.ntiles, cb, x, xs);
+        if constexpr (sizeof(S) == 2) {
+#pragma unroll
+            for (int k = 0; k < 24; ++k) x[k] *= xs;
+        }
         if constexpr (EPI == EPI_G5XPAY) g5_scale<R>(x, epi.g_re, epi.g_im);
 #pragma unroll
         for (int k = 0; k < 24; ++k) acc[k] = fma_(epi.a, acc[k], x[k]);
@@ -245,7 +260,7 @@ dslash_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __restr
 #pragma unroll
         for (int k = 12; k < 24; ++k) acc[k] = -acc[k];
     }
-    store_spinor<R>(out, cb, acc);
+    store_field<S>(out, g.ntiles, cb, acc);
 }
 
 }  // namespace lqcd

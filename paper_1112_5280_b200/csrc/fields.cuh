@@ -14,6 +14,7 @@
 //           recon-12); every link is stored twice (as the forward link of x and the backward link of
 //           x + mu^), which costs capacity, not traffic: one application reads each copy it needs once.
 #pragma once
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
 namespace lqcd {
@@ -100,6 +101,112 @@ __device__ __forceinline__ void recon_row2(R u[18]) {
         u[12 + 2 * c + 1] = -im;
     }
 }
+
+// ---- 16-bit storage (next row f4; "RECONSTRUCT TWELVE [3]" and the half-precision storage of ref. [3],
+// PAPER.md:89, :139): fields are stored as IEEE half, the arithmetic stays fp32 --------------------------------
+//   half spinor: 24 halfs = 3 16-byte words per site, [tile][q 3][32] as above, holding v / n(x) with
+//                n(x) = max_k |v_k(x)| (so every stored number is in [-1, 1] and the 11-bit significand is
+//                relative to the site's largest component); the fp32 norms n(x) follow the words of all tiles:
+//                float[32 ntiles] at byte offset 48 * 32 * ntiles.  52 bytes per site.
+//   links:       12-real storage only, 3 8-byte words of 4 halfs, [p][tile][hop 8][w 3][32]; entries of an SU(3)
+//                matrix are in [-1, 1] already.  24 bytes per link.
+constexpr int HALF_Q = 3;  // 16-byte words per half-precision spinor
+
+__host__ __device__ __forceinline__ size_t half_spinor_words(int ntiles) { return (size_t)HALF_Q * TILE * ntiles; }
+
+__device__ __forceinline__ void unpack_h8(const uint4& w, float* v) {
+    const __half2* h = reinterpret_cast<const __half2*>(&w);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float2 f = __half22float2(h[i]);
+        v[2 * i] = f.x;
+        v[2 * i + 1] = f.y;
+    }
+}
+
+// v = the stored (normalised) components, n = the site norm: the spinor is n * v.  The dslash kernel never
+// forms n * v: the hop is linear, so n rides on the accumulation factor of step K5.
+__device__ __forceinline__ void load_spinor_h(const __half* __restrict__ base, int ntiles, int cb, float v[24], float& n) {
+    const uint4* words = reinterpret_cast<const uint4*>(base);
+    const uint4* p = words + (size_t)(cb / TILE) * (HALF_Q * TILE) + (cb % TILE);
+    n = __ldg(reinterpret_cast<const float*>(words + half_spinor_words(ntiles)) + cb);
+#pragma unroll
+    for (int q = 0; q < HALF_Q; ++q) {
+        const uint4 w = __ldg(p + q * TILE);
+        unpack_h8(w, v + 8 * q);
+    }
+}
+
+__device__ __forceinline__ void store_spinor_h(__half* __restrict__ base, int ntiles, int cb, const float v[24]) {
+    uint4* words = reinterpret_cast<uint4*>(base);
+    uint4* p = words + (size_t)(cb / TILE) * (HALF_Q * TILE) + (cb % TILE);
+    float n = 0.f;
+#pragma unroll
+    for (int k = 0; k < 24; ++k) n = fmaxf(n, fabsf(v[k]));
+    const float inv = n > 0.f ? 1.f / n : 0.f;
+#pragma unroll
+    for (int q = 0; q < HALF_Q; ++q) {
+        uint4 w;
+        __half2* h = reinterpret_cast<__half2*>(&w);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) h[i] = __floats2half2_rn(v[8 * q + 2 * i] * inv, v[8 * q + 2 * i + 1] * inv);
+        p[q * TILE] = w;
+    }
+    reinterpret_cast<float*>(words + half_spinor_words(ntiles))[cb] = n;
+}
+
+// word 0 of hop k's link of site cb (parity p) in the half-precision link field, in 8-byte words
+__host__ __device__ __forceinline__ size_t link_word0_h(int ntiles, int p, int cb, int k) {
+    return ((size_t)(p * ntiles + cb / TILE) * 8 + k) * (3 * TILE) + (cb % TILE);
+}
+
+__device__ __forceinline__ void load_link_h(const uint2* __restrict__ site_links, int k, float u[18]) {
+#pragma unroll
+    for (int w = 0; w < 3; ++w) {
+        const uint2 x = __ldcs(site_links + (k * 3 + w) * TILE);
+        const __half2* h = reinterpret_cast<const __half2*>(&x);
+        const float2 a = __half22float2(h[0]), b = __half22float2(h[1]);
+        u[4 * w] = a.x; u[4 * w + 1] = a.y; u[4 * w + 2] = b.x; u[4 * w + 3] = b.y;
+    }
+    recon_row2<float>(u);
+}
+
+// Storage type S -> arithmetic type, and uniform field access for the kernels (ntiles is only used by half).
+template <typename S> struct Compute { using type = S; };
+template <> struct Compute<__half> { using type = float; };
+
+// the spinor at cb is scale * v (scale = 1 for fp32 / fp64 storage)
+template <typename S>
+__device__ __forceinline__ void load_field(const S* __restrict__ base, int ntiles, int cb, typename Compute<S>::type v[24],
+                                           typename Compute<S>::type& scale) {
+    if constexpr (sizeof(S) == 2) {
+        load_spinor_h(base, ntiles, cb, v, scale);
+    } else {
+        load_spinor<S>(base, cb, v);
+        scale = 1;
+    }
+}
+template <typename S>
+__device__ __forceinline__ void store_field(S* __restrict__ base, int ntiles, int cb, const typename Compute<S>::type v[24]) {
+    if constexpr (sizeof(S) == 2) store_spinor_h(base, ntiles, cb, v); else store_spinor<S>(base, cb, v);
+}
+// elements of S between the even and the odd half of a native full spinor
+template <typename S>
+__host__ __device__ __forceinline__ size_t half_stride(int ntiles) {
+    return sizeof(S) == 2 ? (size_t)(24 + 2) * TILE * ntiles : (size_t)24 * TILE * ntiles;
+}
+
+// storage-type view of the link field
+template <typename S, int RECON> struct LinkStore {
+    using R = typename Compute<S>::type;
+    using word = typename LinkWord<R, RECON>::type;
+    static __host__ __device__ __forceinline__ size_t word0(int ntiles, int p, int cb, int k) { return link_word0<R, RECON>(ntiles, p, cb, k); }
+};
+template <int RECON> struct LinkStore<__half, RECON> {
+    using R = float;
+    using word = uint2;
+    static __host__ __device__ __forceinline__ size_t word0(int ntiles, int p, int cb, int k) { return link_word0_h(ntiles, p, cb, k); }
+};
 
 // L1 + K2: link of hop k for the site whose hop-0 word-0 address is `site_links`.
 template <typename R, int RECON>

@@ -45,8 +45,12 @@ inline bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
     return a0 < b0 + nb && b0 < a0 + na;
 }
 
-inline size_t elem(const lqcd_ctx* c) { return c->p.precision == 32 ? 4 : 8; }
-inline size_t half_bytes(const lqcd_ctx* c) { return (size_t)24 * TILE * c->g.ntiles * elem(c); }  // padded to whole tiles
+inline size_t elem(const lqcd_ctx* c) { return c->p.precision / 8; }                      // stored element
+inline size_t canon_elem(const lqcd_ctx* c) { return c->p.precision == 64 ? 8 : 4; }       // canonical element (16-bit storage: float)
+// native half spinor, padded to whole tiles; 16-bit storage adds one fp32 norm per site
+inline size_t half_bytes(const lqcd_ctx* c) {
+    return (size_t)TILE * c->g.ntiles * (24 * elem(c) + (c->p.precision == 16 ? 4 : 0));
+}
 inline size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
 constexpr int HOST_SLOTS = 3;  // pipeline depth of lqcd_dslash_eo_host_batch
 
@@ -67,9 +71,10 @@ template <typename R, int RECON, int EPI, bool CBC, int BLOCK>
 lqcd_status launch_block(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
                          const EpiArgs& e, int parity, cudaStream_t st) {
     const dim3 grid((c->g.Vh + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
-    const Epilogue<R> epi{(R)e.a, (R)e.g_re, (R)e.g_im, e.g5_out};
+    using A = typename Compute<R>::type;  // R is the storage type here, A the arithmetic type
+    const Epilogue<A> epi{(A)e.a, (A)e.g_re, (A)e.g_im, e.g5_out};
     dslash_kernel<R, RECON, EPI, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
-        (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<R>(c));
+        (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<A>(c));
     return after_launch();
 }
 
@@ -105,6 +110,7 @@ lqcd_status launch_recon(const lqcd_ctx* c, void* out, const void* gauge, const 
 // out_p = epilogue(H in); parity < 0: both parities, full fields.
 lqcd_status launch_dslash(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
                           const EpiArgs& e, int parity, cudaStream_t st) {
+    if (c->p.precision == 16) return launch_recon<__half, 12>(c, out, gauge, in, xin, e, parity, st);
     if (c->p.precision == 32) {
         return c->p.recon == 12 ? launch_recon<float, 12>(c, out, gauge, in, xin, e, parity, st)
                                 : launch_recon<float, 18>(c, out, gauge, in, xin, e, parity, st);
@@ -126,8 +132,9 @@ extern "C" {
 
 lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p) {
     if (!ctx || !p) return LQCD_EINVAL;
-    if (p->precision != 32 && p->precision != 64) return LQCD_EINVAL;
+    if (p->precision != 16 && p->precision != 32 && p->precision != 64) return LQCD_EINVAL;
     if (p->recon != 12 && p->recon != 18) return LQCD_EINVAL;
+    if (p->precision == 16 && p->recon != 12) return LQCD_EUNSUPPORTED;  // 16-bit storage: 12-real links only
     double vol = 1;
     bool cbc = false;
     for (int mu = 0; mu < 4; ++mu) {
@@ -167,7 +174,7 @@ size_t lqcd_workspace_bytes(const lqcd_ctx* c) { return c ? half_bytes(c) : 0; }
 
 size_t lqcd_host_workspace_bytes(const lqcd_ctx* c) {
     if (!c) return 0;
-    const size_t canon_gauge = (size_t)4 * 2 * c->g.Vh * 18 * elem(c);
+    const size_t canon_gauge = (size_t)4 * 2 * c->g.Vh * 18 * canon_elem(c);
     return align256(lqcd_gauge_bytes(c)) + align256(canon_gauge) + HOST_SLOTS * 4 * align256(half_bytes(c));
 }
 
@@ -184,7 +191,9 @@ lqcd_status lqcd_pack_gauge(const lqcd_ctx* c, void* native, const void* canon, 
     if (!aligned16(native) || !aligned16(canon)) return LQCD_EALIGN;
     const dim3 grid((c->g.Vh + 127) / 128, 8, 2);
     cudaStream_t st = (cudaStream_t)stream;
-    if (c->p.precision == 32) {
+    if (c->p.precision == 16) {
+        pack_gauge_h_kernel<<<grid, 128, 0, st>>>((__half*)native, (const float*)canon, c->g);
+    } else if (c->p.precision == 32) {
         if (c->p.recon == 12) pack_gauge_kernel<float, 12><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);
         else pack_gauge_kernel<float, 18><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);
     } else {
@@ -200,7 +209,10 @@ static lqcd_status pack_unpack(const lqcd_ctx* c, void* dst, const void* src, in
     if (!aligned16(dst) || !aligned16(src)) return LQCD_EALIGN;
     const dim3 grid((c->g.Vh + 127) / 128, parity < 0 ? 2 : 1);
     cudaStream_t st = (cudaStream_t)stream;
-    if (c->p.precision == 32) {
+    if (c->p.precision == 16) {
+        if (unpack) pack_spinor_h_kernel<true><<<grid, 128, 0, st>>>(dst, src, c->g, parity);
+        else pack_spinor_h_kernel<false><<<grid, 128, 0, st>>>(dst, src, c->g, parity);
+    } else if (c->p.precision == 32) {
         if (unpack) pack_spinor_kernel<float, true><<<grid, 128, 0, st>>>((float*)dst, (const float*)src, c->g, parity);
         else pack_spinor_kernel<float, false><<<grid, 128, 0, st>>>((float*)dst, (const float*)src, c->g, parity);
     } else {
@@ -384,6 +396,7 @@ lqcd_status lqcd_cg_solve_tm(const lqcd_ctx* c, void* x, const void* gauge, cons
     const size_t hb = c ? half_bytes(c) : 0;
     lqcd_status s = check_fields(c, x, gauge, b, hb);
     if (s != LQCD_OK) return s;
+    if (c->p.precision == 16) return LQCD_EUNSUPPORTED;  // the solver's vectors are fp32 / fp64
     if (!workspace || !(tol > 0.0) || maxiter < 0) return LQCD_EINVAL;
     if (reinterpret_cast<uintptr_t>(workspace) & 255u) return LQCD_EALIGN;
     const size_t wb = lqcd_cg_workspace_bytes(c);
@@ -487,8 +500,8 @@ lqcd_status lqcd_dslash_eo_host_batch(const lqcd_ctx* c, int n, void* const* out
     if (reinterpret_cast<uintptr_t>(ws) & 255u) return LQCD_EALIGN;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t hb = half_bytes(c);                             // native half spinor (padded to whole tiles)
-    const size_t cb_bytes = (size_t)24 * c->g.Vh * elem(c);     // canonical half spinor
-    const size_t canon_gauge = (size_t)4 * 2 * c->g.Vh * 18 * elem(c);
+    const size_t cb_bytes = (size_t)24 * c->g.Vh * canon_elem(c);     // canonical half spinor
+    const size_t canon_gauge = (size_t)4 * 2 * c->g.Vh * 18 * canon_elem(c);
     char* base = static_cast<char*>(ws);
     char* g_nat = base;                 base += align256(lqcd_gauge_bytes(c));
     char* g_can = base;                 base += align256(canon_gauge);

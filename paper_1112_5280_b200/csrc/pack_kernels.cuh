@@ -74,4 +74,47 @@ __global__ void pack_spinor_kernel(R* __restrict__ dst_, const R* __restrict__ s
     }
 }
 
+// ---- 16-bit storage: canonical complex64 <-> native half (fields.cuh) ------------------------------------
+
+// 12-real links only.  grid: (ceil(Vh / block), 8 hops, 2 parities).
+__global__ void pack_gauge_h_kernel(__half* __restrict__ native, const float* __restrict__ canon, Geom g) {
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= g.Vh) return;
+    const int k = blockIdx.y, p = blockIdx.z, mu = k >> 1;
+    const size_t V = (size_t)2 * g.Vh;
+    const size_t site = (k & 1) ? lex_back(g, cb, p, mu) : lex_of(g, cb, p);
+    const float* src = canon + ((size_t)mu * V + site) * 18;
+    __half* dst = native + link_word0_h(g.ntiles, p, cb, k) * 4;
+#pragma unroll
+    for (int w = 0; w < 3; ++w)
+#pragma unroll
+        for (int l = 0; l < 4; ++l) dst[(size_t)w * TILE * 4 + l] = __float2half_rn(src[w * 4 + l]);
+}
+
+// mode as in pack_spinor_kernel; the canonical side is complex64
+template <bool UNPACK>
+__global__ void pack_spinor_h_kernel(void* __restrict__ dst_, const void* __restrict__ src_, Geom g, int mode) {
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= g.Vh) return;
+    size_t canon_site = (size_t)cb, native_off = 0;
+    if (mode < 0) {
+        const int p = blockIdx.y;
+        canon_site = lex_of(g, cb, p);
+        native_off = (size_t)p * half_stride<__half>(g.ntiles);
+    }
+    float v[24];
+    if (UNPACK) {
+        float n;
+        load_spinor_h(static_cast<const __half*>(src_) + native_off, g.ntiles, cb, v, n);
+        float* can = static_cast<float*>(dst_) + canon_site * 24;
+#pragma unroll
+        for (int k = 0; k < 24; ++k) can[k] = v[k] * n;
+    } else {
+        const float* can = static_cast<const float*>(src_) + canon_site * 24;
+#pragma unroll
+        for (int k = 0; k < 24; ++k) v[k] = can[k];
+        store_spinor_h(static_cast<__half*>(dst_) + native_off, g.ntiles, cb, v);
+    }
+}
+
 }  // namespace lqcd

@@ -13,7 +13,7 @@ from lattice_inputs import parity_mask
 
 
 def cdtype(precision):
-    return np.complex64 if precision == 32 else np.complex128
+    return np.complex128 if precision == 64 else np.complex64  # precision 16 exchanges complex64
 
 
 def half_of(psi_full: np.ndarray, dims, parity: int) -> np.ndarray:

@@ -241,3 +241,57 @@ def test_host_batch_pipeline_matches_device_path(H, dims):
     g.ctx.dslash_eo_host_batch(outs2, None, ins, par, ws)
     assert all(np.array_equal(a.numpy(), b.numpy()) for a, b in zip(outs, outs2))
     g.ctx.dslash_eo_host_batch([], None, [], [], ws)  # empty batch is a no-op
+
+
+# ------------------------------------------------------------------ next row f4: 16-bit storage
+TOL16 = 2e-3   # 4 x 2^-11: DESIGN.md section 7 (inputs, links and output each rounded to an 11-bit significand)
+
+
+def _quantise_spinor(psi):
+    """What precision 16 stores: components / site max rounded to IEEE half, times the fp32 site max (numpy emulation
+    of the storage format only; no arithmetic of the method)."""
+    v = np.ascontiguousarray(psi.astype(np.complex64)).view(np.float32).reshape(*psi.shape[:-2], 24)
+    n = np.abs(v).max(axis=-1, keepdims=True)
+    inv = np.where(n > 0, np.float32(1) / np.where(n > 0, n, 1), 0).astype(np.float32)
+    q = (v * inv).astype(np.float16).astype(np.float32) * n
+    return q.reshape(*psi.shape[:-2], 4, 6).view(np.complex64).reshape(psi.shape)
+
+
+def _quantise_links(U):
+    """First two rows rounded to half; the third row is what conj(row0 x row1) rebuilds from them (fp64 here)."""
+    r = np.ascontiguousarray(U.astype(np.complex64)).view(np.float32).astype(np.float16).astype(np.float32)
+    Uq = r.view(np.complex64).reshape(U.shape).astype(np.complex128)
+    Uq[..., 2, :] = np.conj(np.cross(Uq[..., 0, :], Uq[..., 1, :]))
+    return Uq
+
+
+@pytest.mark.parametrize("dims,bc", [((8, 8, 8, 16), (1, 1, 1, -1)), ((6, 6, 6, 6), tuple(np.exp(1j * np.array([0.3, -1.1, 2.0, np.pi]))))])
+def test_half_precision_storage(H, dims, bc):
+    U = li.random_su3_links(dims, seed=91).astype(np.complex64)
+    psi = li.gaussian_spinor(dims, seed=92).astype(np.complex64)
+    psi *= np.exp(np.random.default_rng(93).uniform(-6, 6, size=dims[::-1]))[..., None, None].astype(np.float32)  # site norms over 5 decades
+    g = H.Gpu(dims, 16, 12, bc, U)
+    # storage round trip is exactly the emulated quantisation
+    assert np.array_equal(g.from_native(g.to_native(psi, -1), -1), _quantise_spinor(psi))
+    Uq, psiq = _quantise_links(U), _quantise_spinor(psi)
+    for op in (0, 1):
+        got = g.dslash_eo(H.half_of(psi, dims, 1 - op), op)
+        ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, op), dims, op)
+        assert H.rel_l2(got, ref) <= TOL16
+        # against the oracle fed the values actually stored: only the output rounding (2^-11 of the site max) is left
+        refq = H.half_of(oracle.dslash_eo(Uq, psiq, dims, bc, op), dims, op)
+        assert H.rel_l2(got, refq) <= 6e-4
+        assert H.rel_l2(got, _quantise_spinor(refq.astype(np.complex64))) <= 2e-4   # up to ties at rounding boundaries
+    assert H.rel_l2(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc)) <= TOL16
+    refM = H.half_of(oracle.apply_M(U, psi, dims, bc, 0.15, 1), dims, 0)
+    assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), 0.15, 1), refM) <= TOL16
+    refT = H.half_of(oracle.apply_M_tm(U, psi, dims, bc, 0.15, 0.3, 1), dims, 0)
+    assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), 0.15, 1, mu=0.3), refT) <= TOL16
+    assert H.rel_l2(g.apply_M(psi, 0.15, 0, mu=-0.2), oracle.apply_M_tm(U, psi, dims, bc, 0.15, -0.2, 0)) <= TOL16
+    # a zero site stays zero (norm 0), and the solver entry points refuse 16-bit contexts
+    z = np.zeros_like(H.half_of(psi, dims, 1))
+    assert not g.dslash_eo(z, 0).any()
+    import torch, paper_1112_5280_b200 as L
+    with pytest.raises(L.LqcdError) as e:
+        g.ctx.cg_solve_tm(g.buf(), g.gauge, g.buf(), 0.1, 0.1, 1e-3, 5, torch.empty(1 << 20, dtype=torch.uint8, device="cuda:0"))
+    assert e.value.status == L.LQCD_EUNSUPPORTED
