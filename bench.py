@@ -53,7 +53,7 @@ def parse_args():
     ap.add_argument("--block", type=int, default=0, help="dslash block size override (tuning)")
     ap.add_argument("--chain", action="store_true", help="also time config 5: apply_M(eo=1) x100 chained at 48^3x96")
     ap.add_argument("--no-extras", action="store_true", help="skip the fp64 / chain / e2e / cpu legs (profiling runs)")
-    ap.add_argument("--legs", default="all", help="comma list of extra legs to run: matrix,cg,e2e,other,cgmixed,cpu (default all)")
+    ap.add_argument("--legs", default="all", help="comma list of extra legs to run: matrix,cg,e2e,other,fp16,cgmixed,cpu (default all)")
     return ap.parse_args()
 
 
@@ -144,7 +144,7 @@ class Workload:
         c = li.CONFIGS[cfg_id]
         self.cfg_id, self.dims, self.bc, self.kappa = cfg_id, c["dims"], c["bc"], c["kappa"]
         self.precision, self.recon, self.dev, self.nbuf = precision, recon, dev, nbuf
-        cd = np.complex64 if precision == 32 else np.complex128
+        cd = np.complex128 if precision == 64 else np.complex64  # precision 16 exchanges complex64
         self.ctx = L.Context(self.dims, precision, recon, self.bc)
         if block:
             self.ctx.set_block_threads(block)
@@ -180,7 +180,9 @@ class Workload:
         return self.nbuf * self.Vh
 
     def bytes_per_launch(self):
-        return REALS_PER_SITE[self.recon] * (self.precision // 8) * self.Vh
+        # 16-bit storage: 24 halfs + one fp32 norm per spinor site (in and out), 12 halfs per link
+        per_site = 2 * 52 + 8 * 24 if self.precision == 16 else REALS_PER_SITE[self.recon] * (self.precision // 8)
+        return per_site * self.Vh
 
 
 def timed_steps(torch, dist, fn, steps, warmup):
@@ -491,6 +493,13 @@ def run_b200(args):
         line[f"fp{other}"] = {"gflops": r2["gflops"], "achieved_gbs": r2["gbs"], "frac": r2["gbs"] / peak,
                               "frac_of_nominal_8TBs": r2["gbs"] / NOMINAL_HBM_GBS, "us_per_launch": r2["us_per_launch"],
                               "traffic": ncu_traffic(other, args.recon)}
+        if want("fp16") and args.recon == 12:
+            w16 = Workload(args.config, 16, 12, dev, args.block, keep_host=False)
+            r16 = kernel_leg(torch, dist, w16, max(1, args.steps // 2), args.warmup, world)
+            line["fp16_storage"] = {"gflops": r16["gflops"], "achieved_gbs": r16["gbs"], "frac": r16["gbs"] / peak,
+                                    "us_per_launch": r16["us_per_launch"],
+                                    "model": "296 B per site: 2 x (24 halfs + fp32 norm) + 8 x 12 halfs; fp32 arithmetic"}
+            del w16
         if rank == 0 and want("cgmixed"):
             w64, w32 = (w2, w) if other == 64 else (w, w2)
             line["cg_fp64"] = cg_leg(torch, w64, tol=1e-10)
