@@ -295,3 +295,42 @@ def test_half_precision_storage(H, dims, bc):
     with pytest.raises(L.LqcdError) as e:
         g.ctx.cg_solve_tm(g.buf(), g.gauge, g.buf(), 0.1, 0.1, 1e-3, 5, torch.empty(1 << 20, dtype=torch.uint8, device="cuda:0"))
     assert e.value.status == L.LQCD_EUNSUPPORTED
+
+
+@pytest.mark.parametrize("precision", [16, 32, 64])
+def test_no_writes_outside_the_declared_buffer_sizes(H, precision):
+    """Every output / workspace buffer is carved out of a larger allocation filled with a canary byte; after the
+    hot-path calls on a lattice with a ragged last tile, everything outside the declared sizes is untouched."""
+    import torch
+    dims, bc = (6, 6, 6, 6), (1, 1, 1, -1)
+    U = li.random_su3_links(dims, seed=95).astype(H.cdtype(precision))
+    psi = li.gaussian_spinor(dims, seed=96).astype(H.cdtype(precision))
+    g = H.Gpu(dims, precision, 12, bc, U)
+    G = 4096
+    def guarded(nbytes):
+        big = torch.full((nbytes + 2 * G,), 0xAB, dtype=torch.uint8, device="cuda:0")
+        return big, big[G:G + nbytes]
+    def intact(big, nbytes):
+        return bool((big[:G] == 0xAB).all() and (big[G + nbytes:] == 0xAB).all())
+    hb, fb = g.ctx.spinor_bytes(True), g.ctx.spinor_bytes(False)
+    bo, out = guarded(hb); bw, ws = guarded(g.ctx.workspace_bytes()); bf, outf = guarded(fb)
+    in_e, in_o, in_f = g.to_native(H.half_of(psi, dims, 0), 0), g.to_native(H.half_of(psi, dims, 1), 1), g.to_native(psi, -1)
+    g.ctx.dslash_eo(out, g.gauge, in_o, 0)
+    g.ctx.dslash_eo(out, g.gauge, in_e, 1)
+    g.ctx.apply_M(out, g.gauge, in_e, 0.13, 1, ws)
+    g.ctx.apply_M_tm(out, g.gauge, in_e, 0.13, 0.2, 1, ws)
+    g.ctx.dslash_full(outf, g.gauge, in_f)
+    g.ctx.apply_M_tm(outf, g.gauge, in_f, 0.13, 0.2, 0, None)
+    torch.cuda.synchronize()
+    assert intact(bo, hb) and intact(bw, g.ctx.workspace_bytes()) and intact(bf, fb)
+    if precision != 16:
+        bc_, cws = guarded(g.ctx.cg_workspace_bytes())
+        g.ctx.cg_solve_tm(out, g.gauge, in_e, 0.13, 0.2, 1e-4, 50, cws)
+        assert intact(bo, hb) and intact(bc_, g.ctx.cg_workspace_bytes())
+    # pack / unpack stay inside their buffers too
+    bp, nat = guarded(fb)
+    g.ctx.pack_spinor(nat, torch.from_numpy(psi).to("cuda:0"), -1)
+    bg, gn = guarded(g.ctx.gauge_bytes())
+    g.ctx.pack_gauge(gn, torch.from_numpy(np.ascontiguousarray(U)).to("cuda:0"))
+    torch.cuda.synchronize()
+    assert intact(bp, fb) and intact(bg, g.ctx.gauge_bytes())
