@@ -20,8 +20,8 @@
  *     (PyTorch) allocates and frees every buffer; the library allocates no field memory and
  *     keeps no pointer after a call returns.  lqcd_ctx is host memory owned by the library.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
- *     entry points only enqueue work and return; they never synchronise.  The *_host entry
- *     point synchronises `stream` before returning (its results live in host memory).
+ *     entry points only enqueue work and return; they never synchronise.  The *_host entry points
+ *     and the CG solvers synchronise `stream` before returning (their results live in host memory).
  *   - All device field pointers must be 16-byte aligned (LQCD_EALIGN otherwise).
  *   - The stencil is not in-place safe: `out` overlapping `in` / `workspace` gives LQCD_EALIAS.
  *   - Errors are return codes only: nothing throws, aborts or prints.

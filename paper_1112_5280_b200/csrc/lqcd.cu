@@ -1,6 +1,7 @@
 // lqcd.cu -- host side of the C ABI declared in include/lqcd.h: argument checks, template
-// dispatch (precision x recon x xpay x bc kind x block size) and kernel launches.
-// No field memory is allocated here and nothing synchronises except lqcd_dslash_eo_host.
+// dispatch (storage precision x recon x epilogue x bc kind x block size), kernel launches, the CG
+// loops and the pipelined host-buffer path.  No field memory is allocated here; only the entry points
+// that return results to host memory (lqcd_dslash_eo_host*, lqcd_cg_solve_tm*) synchronise.
 #include "../../include/lqcd.h"
 
 #include <atomic>
