@@ -105,3 +105,38 @@ def test_config5_chain_per_step_parity(cfg5, recon):
             assert H.rel_l2(got[idx], ref) <= TOL[32], k
         x, y = y, x
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_config4_properties_at_full_size(cfg4, precision):
+    """Properties that hold at any size, checked on the GPU at 32^3x64 with the bench's launch configuration:
+    gamma5-hermiticity <phi_e, H_eo psi_o> = <g5 H_oe g5 phi_e, psi_o> (pin P3), linearity, and
+    Q(mu)^dagger = Q(-mu) for the twisted-mass operator the solver iterates with."""
+    import torch
+    import gpu_harness as H
+    c, U64, psi64 = cfg4
+    dims, bc = c["dims"], c["bc"]
+    cd = H.cdtype(precision)
+    g = H.Gpu(dims, precision, 12, bc, U64.astype(cd))
+    phi = li.gaussian_spinor(dims, seed=77).astype(cd)
+    g5 = np.array([1, 1, -1, -1], dtype=np.float64)[:, None]
+    psi_o, phi_e = H.half_of(psi64.astype(cd), dims, 1), H.half_of(phi, dims, 0)
+    lhs = np.vdot(phi_e.astype(np.complex128), g.dslash_eo(psi_o, 0).astype(np.complex128))
+    rhs = np.vdot((g5 * g.dslash_eo((g5 * phi_e).astype(cd), 1)).astype(np.complex128), psi_o.astype(np.complex128))
+    tol = 1e-12 if precision == 64 else 2e-6
+    assert abs(lhs - rhs) <= tol * abs(lhs)
+    # linearity
+    a, b = 0.7 - 0.2j, -1.3 + 0.4j
+    psi2 = H.half_of(li.gaussian_spinor(dims, seed=78).astype(cd), dims, 1)
+    comb = g.dslash_eo((a * psi_o + b * psi2).astype(cd), 0)
+    assert H.rel_l2(comb, a * g.dslash_eo(psi_o, 0).astype(np.complex128) + b * g.dslash_eo(psi2, 0).astype(np.complex128)) <= TOL[precision]
+    # <phi, Q(mu) psi> = <Q(-mu) phi, psi> on even fields
+    kappa, mu = c["kappa"], 0.05
+    psi_e = H.half_of(psi64.astype(cd), dims, 0)
+    def Q(v, m):
+        out = g.buf()
+        g.ctx.apply_Q_tm(out, g.gauge, g.to_native(v, 0), kappa, m, g.buf())
+        return g.from_native(out, 0).astype(np.complex128)
+    l2 = np.vdot(phi_e.astype(np.complex128), Q(psi_e, mu))
+    r2 = np.vdot(Q(phi_e, -mu), psi_e.astype(np.complex128))
+    assert abs(l2 - r2) <= tol * abs(l2)
