@@ -116,6 +116,21 @@ lqcd_status lqcd_dslash_full(const lqcd_ctx* ctx, void* out_dev, const void* gau
 lqcd_status lqcd_dslash_eo(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
                            int out_parity, void* stream);
 
+/* Time-slab decomposition primitives (next row f3; the paper's multi-device story is host-mediated,
+ * PAPER.md:71, :103; here: T slabs with ghost time slices).  A rank holds T_loc global time slices as a local
+ * lattice of T = T_loc + 2 slices whose slices 0 and T_loc + 1 are ghosts, filled by the caller with plain copies
+ * of the neighbours' boundary slices: in the native layout a time slice of a half spinor is the contiguous
+ * byte range [t, t + 1) * lqcd_time_slice_bytes(ctx) (0 = not available: slice not made of whole tiles, or
+ * precision 16).  lqcd_dslash_eo_range computes only the output sites with t in [t_begin, t_end) (interior
+ * slices 1..T_loc; or interior first, boundary slices after the exchange).  lqcd_set_time_slab moves the
+ * t boundary phase from the local wrap to where the global boundary cuts the slab: the forward hop from slice
+ * t_cross_fwd and the backward hop from slice t_cross_bwd carry bc_t / conj(bc_t); -1 = none; the defaults of a
+ * whole lattice are (T - 1, 0).  Links need no exchange: each rank packs the links of its slices, ghosts included. */
+lqcd_status lqcd_set_time_slab(lqcd_ctx* ctx, int t_cross_fwd, int t_cross_bwd);
+lqcd_status lqcd_dslash_eo_range(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
+                                 int out_parity, int t_begin, int t_end, void* stream);
+size_t lqcd_time_slice_bytes(const lqcd_ctx* ctx);
+
 /* eo = 0: out = in - kappa H in, native full spinors, one launch, workspace unused (may be NULL).
  * eo = 1: out_e = in_e - kappa^2 H_eo H_oe in_e, native even half spinors; two launches;
  *         workspace_dev holds the intermediate odd half spinor (lqcd_workspace_bytes). */

@@ -18,7 +18,7 @@ PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, -1
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
-    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_dslash_eo_host_batch", "lqcd_launch_count",
+    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_set_time_slab", "lqcd_dslash_eo_range", "lqcd_time_slice_bytes", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_dslash_eo_host_batch", "lqcd_launch_count",
     "lqcd_set_block_threads", "lqcd_status_string", "lqcd_last_cuda_error",
 ]
 
@@ -62,6 +62,10 @@ def _lib():
         lib.lqcd_dslash_full.argtypes = [vp, vp, vp, vp, vp]
         lib.lqcd_dslash_eo.argtypes = [vp, vp, vp, vp, ci, vp]
         lib.lqcd_apply_M.argtypes = [vp, vp, vp, vp, cd, ci, vp, vp]
+        lib.lqcd_set_time_slab.argtypes = [vp, ci, ci]
+        lib.lqcd_dslash_eo_range.argtypes = [vp, vp, vp, vp, ci, ci, ci, vp]
+        lib.lqcd_time_slice_bytes.argtypes = [vp]
+        lib.lqcd_time_slice_bytes.restype = sz
         lib.lqcd_apply_M_tm.argtypes = [vp, vp, vp, vp, cd, cd, ci, vp, vp]
         lib.lqcd_apply_Q_tm.argtypes = [vp, vp, vp, vp, cd, cd, vp, vp]
         lib.lqcd_cg_mixed_workspace_bytes.argtypes = [vp, vp]
@@ -154,6 +158,15 @@ class Context:
     def dslash_eo(self, out, gauge, inp, out_parity, stream=None):
         _chk(_lib().lqcd_dslash_eo(self._h, _ptr(out), _ptr(gauge), _ptr(inp), int(out_parity), _stream(stream)),
              "lqcd_dslash_eo")
+
+    def set_time_slab(self, t_cross_fwd, t_cross_bwd):
+        _chk(_lib().lqcd_set_time_slab(self._h, int(t_cross_fwd), int(t_cross_bwd)), "lqcd_set_time_slab")
+
+    def dslash_eo_range(self, out, gauge, inp, out_parity, t_begin, t_end, stream=None):
+        _chk(_lib().lqcd_dslash_eo_range(self._h, _ptr(out), _ptr(gauge), _ptr(inp), int(out_parity), int(t_begin),
+                                         int(t_end), _stream(stream)), "lqcd_dslash_eo_range")
+
+    def time_slice_bytes(self): return _lib().lqcd_time_slice_bytes(self._h)
 
     def apply_M(self, out, gauge, inp, kappa, eo, workspace=None, stream=None):
         _chk(_lib().lqcd_apply_M(self._h, _ptr(out), _ptr(gauge), _ptr(inp), float(kappa), int(eo),

@@ -199,7 +199,8 @@ __device__ __forceinline__ void g5_scale(R v[24], R g_re, R g_im) {
 template <typename S, int RECON, int EPI, bool CBC, int BLOCK>
 __global__ void __launch_bounds__(BLOCK, MinBlocks<S, RECON>::value * 64 / BLOCK)
 dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restrict__ in, const S* __restrict__ xin,
-              Epilogue<typename Compute<S>::type> epi, Geom g, int parity0, BcPhases<typename Compute<S>::type> bc) {
+              Epilogue<typename Compute<S>::type> epi, Geom g, int parity0, BcPhases<typename Compute<S>::type> bc,
+              int cb_begin, int cb_end) {
     using R = typename Compute<S>::type;
     constexpr bool XPAY = EPI == EPI_XPAY || EPI == EPI_G5XPAY;
     int p = parity0;
@@ -210,8 +211,8 @@ dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restr
         out += (size_t)p * half;
         if (XPAY) xin += (size_t)p * half;
     }
-    const int cb = blockIdx.x * BLOCK + threadIdx.x;
-    if (cb >= g.Vh) return;
+    const int cb = cb_begin + blockIdx.x * BLOCK + threadIdx.x;  // [cb_begin, cb_end): all sites, or a range of time slices
+    if (cb >= cb_end) return;
     const Site s = decode_site(g, cb, p);
 
     // K1: all eight neighbours and boundary-crossing flags

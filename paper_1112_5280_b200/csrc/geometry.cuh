@@ -15,6 +15,8 @@ struct Geom {
     int Vh;          // X*Y*Z*T / 2 (sites per parity)
     int ntiles;      // ceil(Vh / 32): 32-site tiles per parity in the native layout (fields.cuh)
     int sy, sz, st;  // cb strides of y, z, t: Xh, Xh*Y, Xh*Y*Z
+    int tcf, tcb;    // t whose forward / backward hop carries the boundary phase: T-1 / 0 on a whole lattice; a
+                     // time slab (lqcd_set_time_slab) moves them to where the global boundary cuts it, or -1
 };
 
 struct Site {
@@ -69,12 +71,13 @@ __device__ __forceinline__ int neighbour(const Geom& g, int cb, const Site& s, b
             return cross ? cb + (g.Z - 1) * g.sz : cb - g.sz;
         }
     } else {
+        // the wrap decides the address, tcf / tcb decide where the boundary phase sits (the two differ on a time slab)
         if (FWD) {
-            cross = (s.t == g.T - 1);
-            return cross ? cb - (g.T - 1) * g.st : cb + g.st;
+            cross = (s.t == g.tcf);
+            return (s.t == g.T - 1) ? cb - (g.T - 1) * g.st : cb + g.st;
         } else {
-            cross = (s.t == 0);
-            return cross ? cb + (g.T - 1) * g.st : cb - g.st;
+            cross = (s.t == g.tcb);
+            return (s.t == 0) ? cb + (g.T - 1) * g.st : cb - g.st;
         }
     }
 }

@@ -68,56 +68,60 @@ BcPhases<R> make_bc(const lqcd_ctx* c) {
 // epilogue of one launch: mode (EPI_*) and its constants, in double until the kernel's precision is known
 struct EpiArgs { int mode; double a, g_re, g_im; int g5_out; };
 
+// range of checkerboard indices one launch covers: everything, or the time slices [t_begin, t_end)
+struct CbRange { int begin, end; };
+inline CbRange all_sites(const lqcd_ctx* c) { return CbRange{0, c->g.Vh}; }
+
 template <typename R, int RECON, int EPI, bool CBC, int BLOCK>
 lqcd_status launch_block(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                         const EpiArgs& e, int parity, cudaStream_t st) {
-    const dim3 grid((c->g.Vh + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
+                         const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
+    const dim3 grid((rg.end - rg.begin + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
     using A = typename Compute<R>::type;  // R is the storage type here, A the arithmetic type
     const Epilogue<A> epi{(A)e.a, (A)e.g_re, (A)e.g_im, e.g5_out};
     dslash_kernel<R, RECON, EPI, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
-        (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<A>(c));
+        (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<A>(c), rg.begin, rg.end);
     return after_launch();
 }
 
 template <typename R, int RECON, int EPI, bool CBC>
 lqcd_status launch_cbc(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                       const EpiArgs& e, int parity, cudaStream_t st) {
+                       const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
     switch (c->block) {
-        case 64: return launch_block<R, RECON, EPI, CBC, 64>(c, out, gauge, in, xin, e, parity, st);
-        case 128: return launch_block<R, RECON, EPI, CBC, 128>(c, out, gauge, in, xin, e, parity, st);
+        case 64: return launch_block<R, RECON, EPI, CBC, 64>(c, out, gauge, in, xin, e, parity, st, rg);
+        case 128: return launch_block<R, RECON, EPI, CBC, 128>(c, out, gauge, in, xin, e, parity, st, rg);
     }
     return LQCD_EUNSUPPORTED;
 }
 
 template <typename R, int RECON, int EPI>
 lqcd_status launch_epi(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                       const EpiArgs& e, int parity, cudaStream_t st) {
-    return c->complex_bc ? launch_cbc<R, RECON, EPI, true>(c, out, gauge, in, xin, e, parity, st)
-                         : launch_cbc<R, RECON, EPI, false>(c, out, gauge, in, xin, e, parity, st);
+                       const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
+    return c->complex_bc ? launch_cbc<R, RECON, EPI, true>(c, out, gauge, in, xin, e, parity, st, rg)
+                         : launch_cbc<R, RECON, EPI, false>(c, out, gauge, in, xin, e, parity, st, rg);
 }
 
 template <typename R, int RECON>
 lqcd_status launch_recon(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                         const EpiArgs& e, int parity, cudaStream_t st) {
+                         const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
     switch (e.mode) {
-        case EPI_STORE: return launch_epi<R, RECON, EPI_STORE>(c, out, gauge, in, xin, e, parity, st);
-        case EPI_XPAY: return launch_epi<R, RECON, EPI_XPAY>(c, out, gauge, in, xin, e, parity, st);
-        case EPI_G5SCALE: return launch_epi<R, RECON, EPI_G5SCALE>(c, out, gauge, in, xin, e, parity, st);
-        case EPI_G5XPAY: return launch_epi<R, RECON, EPI_G5XPAY>(c, out, gauge, in, xin, e, parity, st);
+        case EPI_STORE: return launch_epi<R, RECON, EPI_STORE>(c, out, gauge, in, xin, e, parity, st, rg);
+        case EPI_XPAY: return launch_epi<R, RECON, EPI_XPAY>(c, out, gauge, in, xin, e, parity, st, rg);
+        case EPI_G5SCALE: return launch_epi<R, RECON, EPI_G5SCALE>(c, out, gauge, in, xin, e, parity, st, rg);
+        case EPI_G5XPAY: return launch_epi<R, RECON, EPI_G5XPAY>(c, out, gauge, in, xin, e, parity, st, rg);
     }
     return LQCD_EUNSUPPORTED;
 }
 
 // out_p = epilogue(H in); parity < 0: both parities, full fields.
 lqcd_status launch_dslash(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                          const EpiArgs& e, int parity, cudaStream_t st) {
-    if (c->p.precision == 16) return launch_recon<__half, 12>(c, out, gauge, in, xin, e, parity, st);
+                          const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
+    if (c->p.precision == 16) return launch_recon<__half, 12>(c, out, gauge, in, xin, e, parity, st, rg);
     if (c->p.precision == 32) {
-        return c->p.recon == 12 ? launch_recon<float, 12>(c, out, gauge, in, xin, e, parity, st)
-                                : launch_recon<float, 18>(c, out, gauge, in, xin, e, parity, st);
+        return c->p.recon == 12 ? launch_recon<float, 12>(c, out, gauge, in, xin, e, parity, st, rg)
+                                : launch_recon<float, 18>(c, out, gauge, in, xin, e, parity, st, rg);
     }
-    return c->p.recon == 12 ? launch_recon<double, 12>(c, out, gauge, in, xin, e, parity, st)
-                            : launch_recon<double, 18>(c, out, gauge, in, xin, e, parity, st);
+    return c->p.recon == 12 ? launch_recon<double, 12>(c, out, gauge, in, xin, e, parity, st, rg)
+                            : launch_recon<double, 18>(c, out, gauge, in, xin, e, parity, st, rg);
 }
 
 lqcd_status check_fields(const lqcd_ctx* c, const void* out, const void* gauge, const void* in, size_t nbytes) {
@@ -156,6 +160,7 @@ lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p) {
     g.Vh = g.Xh * g.Y * g.Z * g.T;
     g.ntiles = (g.Vh + TILE - 1) / TILE;
     g.sy = g.Xh; g.sz = g.Xh * g.Y; g.st = g.Xh * g.Y * g.Z;
+    g.tcf = g.T - 1; g.tcb = 0;
     c->complex_bc = cbc;
     c->block = 64;
     *ctx = c;
@@ -234,7 +239,7 @@ lqcd_status lqcd_unpack_spinor(const lqcd_ctx* c, void* canon, const void* nativ
 lqcd_status lqcd_dslash_full(const lqcd_ctx* c, void* out, const void* gauge, const void* in, void* stream) {
     lqcd_status s = check_fields(c, out, gauge, in, c ? 2 * half_bytes(c) : 0);
     if (s != LQCD_OK) return s;
-    return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0, 0}, -1, (cudaStream_t)stream);
+    return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0, 0}, -1, (cudaStream_t)stream, all_sites(c));
 }
 
 lqcd_status lqcd_dslash_eo(const lqcd_ctx* c, void* out, const void* gauge, const void* in, int out_parity,
@@ -242,7 +247,38 @@ lqcd_status lqcd_dslash_eo(const lqcd_ctx* c, void* out, const void* gauge, cons
     if (out_parity != 0 && out_parity != 1) return LQCD_EINVAL;
     lqcd_status s = check_fields(c, out, gauge, in, c ? half_bytes(c) : 0);
     if (s != LQCD_OK) return s;
-    return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0, 0}, out_parity, (cudaStream_t)stream);
+    return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0, 0}, out_parity, (cudaStream_t)stream, all_sites(c));
+}
+
+// ---- next row f3: time-slab decomposition primitives ------------------------------------------------------
+// A rank of a T-slab decomposition holds the time slices [t0, t0 + T_loc) of the global lattice as a local
+// lattice of T_loc + 2 slices: slice 0 and slice T_loc + 1 are ghosts filled from the neighbouring ranks
+// (plain copies of whole time slices, which are contiguous in the native layout), and only the interior
+// slices are computed.  The boundary phase sits where the global boundary cuts the slab, not at the local wrap.
+lqcd_status lqcd_set_time_slab(lqcd_ctx* c, int t_cross_fwd, int t_cross_bwd) {
+    if (!c) return LQCD_EINVAL;
+    if (t_cross_fwd < -1 || t_cross_fwd >= c->g.T || t_cross_bwd < -1 || t_cross_bwd >= c->g.T) return LQCD_EINVAL;
+    c->g.tcf = t_cross_fwd;
+    c->g.tcb = t_cross_bwd;
+    return LQCD_OK;
+}
+
+lqcd_status lqcd_dslash_eo_range(const lqcd_ctx* c, void* out, const void* gauge, const void* in, int out_parity,
+                                 int t_begin, int t_end, void* stream) {
+    if (out_parity != 0 && out_parity != 1) return LQCD_EINVAL;
+    lqcd_status s = check_fields(c, out, gauge, in, c ? half_bytes(c) : 0);
+    if (s != LQCD_OK) return s;
+    if (t_begin < 0 || t_end > c->g.T || t_begin > t_end) return LQCD_EINVAL;
+    if (t_begin == t_end) return LQCD_OK;
+    return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0, 0}, out_parity, (cudaStream_t)stream,
+                         CbRange{t_begin * c->g.st, t_end * c->g.st});
+}
+
+size_t lqcd_time_slice_bytes(const lqcd_ctx* c) {
+    // bytes of one time slice of a native half spinor; 0 if slices are not whole tiles (or 16-bit storage,
+    // whose norms live apart): then the slab path is not available for this lattice
+    if (!c || c->p.precision == 16 || c->g.st % TILE != 0) return 0;
+    return (size_t)c->g.st * 24 * elem(c);
 }
 
 // Shared body of lqcd_apply_M (theta = 0) and lqcd_apply_M_tm (theta = 2 kappa mu).
@@ -253,7 +289,7 @@ static lqcd_status apply_M_impl(const lqcd_ctx* c, void* out, const void* gauge,
     if (eo == 0) {
         lqcd_status s = check_fields(c, out, gauge, in, c ? 2 * half_bytes(c) : 0);
         if (s != LQCD_OK) return s;
-        return launch_dslash(c, out, gauge, in, in, last, -1, st);  // out = (1 + i theta g5) in - kappa H in
+        return launch_dslash(c, out, gauge, in, in, last, -1, st, all_sites(c));  // out = (1 + i theta g5) in - kappa H in
     }
     const size_t hb = c ? half_bytes(c) : 0;
     lqcd_status s = check_fields(c, out, gauge, in, hb);
@@ -264,9 +300,9 @@ static lqcd_status apply_M_impl(const lqcd_ctx* c, void* out, const void* gauge,
     // tmp_o = (1 + i theta g5)^-1 H_oe in_e, with (1 + i theta g5)^-1 = (1 - i theta g5) / (1 + theta^2)
     const double n = 1.0 / (1.0 + theta * theta);
     const EpiArgs first{twisted ? EPI_G5SCALE : EPI_STORE, 0.0, n, -theta * n, 0};
-    s = launch_dslash(c, workspace, gauge, in, nullptr, first, 1, st);
+    s = launch_dslash(c, workspace, gauge, in, nullptr, first, 1, st, all_sites(c));
     if (s != LQCD_OK) return s;
-    return launch_dslash(c, out, gauge, workspace, in, last, 0, st);  // out_e = (1 + i theta g5) in_e - kappa^2 H_eo tmp_o
+    return launch_dslash(c, out, gauge, workspace, in, last, 0, st, all_sites(c));  // out_e = (1 + i theta g5) in_e - kappa^2 H_eo tmp_o
 }
 
 lqcd_status lqcd_apply_M(const lqcd_ctx* c, void* out, const void* gauge, const void* in, double kappa, int eo,

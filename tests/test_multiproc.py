@@ -53,3 +53,39 @@ def test_reference_arm_runs_on_rank0_only():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
                         "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def _slab_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    from paper_1112_5280_b200.slab import TimeSlab
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        s = TimeSlab((8, 8, 8, 16), 32, 12, (1, 1, 1, -1), rank, world)   # host-only: no CUDA call is made
+        sb = s.slice_bytes
+        f = torch.empty((s.Tl + 2) * sb, dtype=torch.uint8)
+        for tl in range(s.Tl + 2):                       # byte pattern = 16 * rank + local slice; ghosts 255
+            s.slice_view(f, tl).fill_(255 if tl in (0, s.Tl + 1) else 16 * rank + tl)
+        s.exchange(f, dist)
+        out[rank] = (int(s.slice_view(f, 0)[0]), int(s.slice_view(f, 0)[-1]), int(s.slice_view(f, s.Tl + 1)[0]),
+                     int(s.slice_view(f, s.Tl + 1)[-1]), int(s.slice_view(f, 1)[0]), s.time_indices(), s.local_parity(0))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_time_slab_ghost_exchange_world2():
+    """Ring exchange of the time-slab decomposition (paper_1112_5280_b200/slab.py) over gloo on CPU tensors:
+    ghost 0 receives the left neighbour's last interior slice, ghost Tl + 1 the right neighbour's first."""
+    world, port = 2, _free_port()
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_slab_worker, args=(world, port, out), nprocs=world, join=True)
+        res = dict(out)
+    Tl = 8
+    for r in range(2):
+        other = 1 - r
+        g0a, g0b, g1a, g1b, own, tidx, lp = res[r]
+        assert g0a == g0b == 16 * other + Tl      # left neighbour (= the other rank on a ring of 2): its slice Tl
+        assert g1a == g1b == 16 * other + 1       # right neighbour: its slice 1
+        assert own == 16 * r + 1                  # interior untouched
+        assert tidx == [(r * Tl - 1 + k) % 16 for k in range(Tl + 2)] and lp == 1
