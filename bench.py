@@ -135,7 +135,7 @@ class ClockSampler:
 class Workload:
     """Seeded inputs of one config on the device in native layout, plus pinned host copies."""
 
-    def __init__(self, cfg_id, precision, recon, dev, block=0, nbuf=NBUF, keep_host=True, in_parity=None, U=None):
+    def __init__(self, cfg_id, precision, recon, dev, block=0, nbuf=NBUF, keep_host=True, in_parity=None, U=None, link_precision=0):
         import numpy as np
         import torch
         import lattice_inputs as li
@@ -145,7 +145,7 @@ class Workload:
         self.cfg_id, self.dims, self.bc, self.kappa = cfg_id, c["dims"], c["bc"], c["kappa"]
         self.precision, self.recon, self.dev, self.nbuf = precision, recon, dev, nbuf
         cd = np.complex128 if precision == 64 else np.complex64  # precision 16 exchanges complex64
-        self.ctx = L.Context(self.dims, precision, recon, self.bc)
+        self.ctx = L.Context(self.dims, precision, recon, self.bc, link_precision)
         if block:
             self.ctx.set_block_threads(block)
         self.Vh = self.ctx.Vh
@@ -504,6 +504,10 @@ def run_b200(args):
             w64, w32 = (w2, w) if other == 64 else (w, w2)
             line["cg_fp64"] = cg_leg(torch, w64, tol=1e-10)
             line["cg_mixed"] = cg_mixed_leg(torch, w64, w32, tol=1e-10)
+            if args.recon == 12:
+                w32h = Workload(args.config, 32, 12, dev, args.block, keep_host=False, nbuf=1, link_precision=16)
+                line["cg_mixed_half_links"] = cg_mixed_leg(torch, w64, w32h, tol=1e-10)
+                del w32h
         del w2
     del w
     torch.cuda.empty_cache()

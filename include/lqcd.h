@@ -78,6 +78,9 @@ typedef struct {
                          registers as conj(row0 x row1) ("RECONSTRUCT TWELVE") */
     double bc_re[4];  /* boundary phase bc_mu = bc_re + i bc_im, |bc_mu| = 1 within 1e-12; */
     double bc_im[4];  /* periodic (1,0), antiperiodic (-1,0), any U(1) phase allowed        */
+    int link_precision; /* 0: links stored like the spinors.  16 with precision 32 and recon 12: fp32 spinors,
+                           links stored as 12 IEEE halfs (24 instead of 48 bytes per link; the link stream is 2/3 of
+                           the traffic) -- meant for the inner solver of lqcd_cg_solve_tm_mixed */
 } lqcd_params;
 
 #define LQCD_PARITY_EVEN 0

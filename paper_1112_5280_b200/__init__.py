@@ -25,7 +25,7 @@ EXPORTS = [
 
 class lqcd_params(ctypes.Structure):
     _fields_ = [("dims", ctypes.c_int * 4), ("precision", ctypes.c_int), ("recon", ctypes.c_int),
-                ("bc_re", ctypes.c_double * 4), ("bc_im", ctypes.c_double * 4)]
+                ("bc_re", ctypes.c_double * 4), ("bc_im", ctypes.c_double * 4), ("link_precision", ctypes.c_int)]
 
 
 class LqcdError(RuntimeError):
@@ -112,10 +112,10 @@ def _chk(status: int, where: str):
 class Context:
     """Owns one lqcd_ctx.  Methods carry the names of the C entry points minus the prefix."""
 
-    def __init__(self, dims, precision=64, recon=18, bc=(1, 1, 1, -1)):
+    def __init__(self, dims, precision=64, recon=18, bc=(1, 1, 1, -1), link_precision=0):
         p = lqcd_params()
         p.dims[:] = [int(d) for d in dims]
-        p.precision, p.recon = int(precision), int(recon)
+        p.precision, p.recon, p.link_precision = int(precision), int(recon), int(link_precision)
         b = [complex(z) for z in bc]
         p.bc_re[:] = [z.real for z in b]
         p.bc_im[:] = [z.imag for z in b]

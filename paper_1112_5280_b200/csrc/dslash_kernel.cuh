@@ -140,7 +140,7 @@ __device__ __forceinline__ void hop_step(typename Compute<S>::type acc[24],
     constexpr bool FWD = (K & 1) == 0;
     R v[24], u[18], scale;
     load_field<S>(in, ntiles, nb[K], v, scale);
-    if constexpr (sizeof(S) == 2) load_link_h(site_links, K, u); else load_link<R, RECON>(site_links, K, u);
+    if constexpr (half_links<S, RECON>) load_link_h(site_links, K, u); else load_link<R, RECON>(site_links, K, u);
     hop_math<R, CBC, MU, FWD>(acc, v, scale, u, (crossmask >> K) & 1u, bc);
 }
 
@@ -169,6 +169,7 @@ template <> struct MinBlocks<float, 18>  { static constexpr int value = LQCD_MIN
 template <> struct MinBlocks<double, 12> { static constexpr int value = LQCD_MINB_F64_R12; };
 template <> struct MinBlocks<double, 18> { static constexpr int value = LQCD_MINB_F64_R18; };
 template <> struct MinBlocks<__half, 12>  { static constexpr int value = LQCD_MINB_F16_R12; };
+template <> struct MinBlocks<float, RECON_12H> { static constexpr int value = LQCD_MINB_F32_R12; };
 
 // Step K6, the epilogue applied to acc = (H in)(x) before the store (EPI):
 //   EPI_STORE    out = acc                                        lqcd_dslash_*

@@ -207,6 +207,15 @@ template <int RECON> struct LinkStore<__half, RECON> {
     using word = uint2;
     static __host__ __device__ __forceinline__ size_t word0(int ntiles, int p, int cb, int k) { return link_word0_h(ntiles, p, cb, k); }
 };
+// fp32 spinors with the links stored as 12 halfs (lqcd_params.link_precision = 16): the link stream is 2/3 of
+// the traffic, and a 2^-11 perturbation of the links is harmless for the inner solver of a defect correction
+constexpr int RECON_12H = 13;
+template <> struct LinkStore<float, RECON_12H> {
+    using R = float;
+    using word = uint2;
+    static __host__ __device__ __forceinline__ size_t word0(int ntiles, int p, int cb, int k) { return link_word0_h(ntiles, p, cb, k); }
+};
+template <typename S, int RECON> constexpr bool half_links = sizeof(S) == 2 || RECON == RECON_12H;
 
 // L1 + K2: link of hop k for the site whose hop-0 word-0 address is `site_links`.
 template <typename R, int RECON>

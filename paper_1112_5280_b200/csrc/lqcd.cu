@@ -117,6 +117,7 @@ lqcd_status launch_dslash(const lqcd_ctx* c, void* out, const void* gauge, const
                           const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
     if (c->p.precision == 16) return launch_recon<__half, 12>(c, out, gauge, in, xin, e, parity, st, rg);
     if (c->p.precision == 32) {
+        if (c->p.link_precision == 16) return launch_recon<float, RECON_12H>(c, out, gauge, in, xin, e, parity, st, rg);
         return c->p.recon == 12 ? launch_recon<float, 12>(c, out, gauge, in, xin, e, parity, st, rg)
                                 : launch_recon<float, 18>(c, out, gauge, in, xin, e, parity, st, rg);
     }
@@ -140,6 +141,8 @@ lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p) {
     if (p->precision != 16 && p->precision != 32 && p->precision != 64) return LQCD_EINVAL;
     if (p->recon != 12 && p->recon != 18) return LQCD_EINVAL;
     if (p->precision == 16 && p->recon != 12) return LQCD_EUNSUPPORTED;  // 16-bit storage: 12-real links only
+    if (p->link_precision != 0 && p->link_precision != 16 && p->link_precision != p->precision) return LQCD_EINVAL;
+    if (p->link_precision == 16 && (p->precision == 64 || p->recon != 12)) return LQCD_EUNSUPPORTED;
     double vol = 1;
     bool cbc = false;
     for (int mu = 0; mu < 4; ++mu) {
@@ -174,7 +177,8 @@ lqcd_status lqcd_destroy(lqcd_ctx* ctx) {
 
 size_t lqcd_spinor_bytes(const lqcd_ctx* c, int half) { return c ? half_bytes(c) * (half ? 1 : 2) : 0; }
 size_t lqcd_gauge_bytes(const lqcd_ctx* c) {
-    return c ? (size_t)2 * 8 * c->p.recon * TILE * c->g.ntiles * elem(c) : 0;  // [parity][tile][hop 8][recon reals][32]
+    const size_t link_elem = c && c->p.link_precision == 16 ? 2 : (c ? elem(c) : 0);
+    return c ? (size_t)2 * 8 * c->p.recon * TILE * c->g.ntiles * link_elem : 0;  // [parity][tile][hop 8][recon reals][32]
 }
 size_t lqcd_workspace_bytes(const lqcd_ctx* c) { return c ? half_bytes(c) : 0; }
 
@@ -197,7 +201,7 @@ lqcd_status lqcd_pack_gauge(const lqcd_ctx* c, void* native, const void* canon, 
     if (!aligned16(native) || !aligned16(canon)) return LQCD_EALIGN;
     const dim3 grid((c->g.Vh + 127) / 128, 8, 2);
     cudaStream_t st = (cudaStream_t)stream;
-    if (c->p.precision == 16) {
+    if (c->p.precision == 16 || c->p.link_precision == 16) {
         pack_gauge_h_kernel<<<grid, 128, 0, st>>>((__half*)native, (const float*)canon, c->g);
     } else if (c->p.precision == 32) {
         if (c->p.recon == 12) pack_gauge_kernel<float, 12><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);

@@ -32,8 +32,8 @@ def scatter_half(half: np.ndarray, dims, parity: int) -> np.ndarray:
 class Gpu:
     """One context plus the packed gauge field on cuda:0."""
 
-    def __init__(self, dims, precision, recon, bc, U: np.ndarray):
-        self.ctx = L.Context(dims, precision, recon, bc)
+    def __init__(self, dims, precision, recon, bc, U: np.ndarray, link_precision=0):
+        self.ctx = L.Context(dims, precision, recon, bc, link_precision)
         self.dims, self.precision = tuple(dims), precision
         self.cd = cdtype(precision)
         self.dev = torch.device("cuda:0")

@@ -79,8 +79,8 @@ def test_cg_edge_cases():
     assert e.value.status == L.LQCD_EINVAL
 
 
-@pytest.mark.parametrize("recon64,recon32", [(18, 12), (12, 12)])
-def test_mixed_precision_cg(recon64, recon32):
+@pytest.mark.parametrize("recon64,recon32,link32", [(18, 12, 0), (12, 12, 0), (12, 12, 16)])
+def test_mixed_precision_cg(recon64, recon32, link32):
     """lqcd_cg_solve_tm_mixed: fp64-accurate solution from fp32 iterations; compared with the fp64 oracle CG
     and with the mixed-precision oracle (outer correction count)."""
     import gpu_harness as H
@@ -89,7 +89,7 @@ def test_mixed_precision_cg(recon64, recon32):
     even = li.parity_mask(dims, 0)[..., None, None]
     b = li.gaussian_spinor(dims, seed=41) * even
     g64 = H.Gpu(dims, 64, recon64, APBC, U)
-    g32 = H.Gpu(dims, 32, recon32, APBC, U.astype(np.complex64))
+    g32 = H.Gpu(dims, 32, recon32, APBC, U.astype(np.complex64), link_precision=link32)  # 16: inner operator with half links
     x = g64.buf()
     ws = torch.empty(g64.ctx.cg_mixed_workspace_bytes(g32.ctx), dtype=torch.uint8, device=g64.dev)
     it, outer, res = g64.ctx.cg_solve_tm_mixed(g32.ctx, x, g64.gauge, g32.gauge, g64.to_native(H.half_of(b, dims, 0), 0),
@@ -100,7 +100,10 @@ def test_mixed_precision_cg(recon64, recon32):
     x_ref, it_ref, _ = cg_oracle.cg_solve_tm(U, b, dims, APBC, kappa, mu, tol, 500)
     assert np.linalg.norm(xg - x_ref) <= 100 * tol * np.linalg.norm(x_ref)
     _, it_mix, outer_mix, _ = cg_oracle.cg_mixed_solve_tm(U, b, dims, APBC, kappa, mu, tol, 1e-4, 2000)
-    assert abs(outer - outer_mix) <= 1 and abs(it - it_mix) <= max(3, it_mix // 10), (it, it_mix, outer, outer_mix)
+    if link32 == 0:
+        assert abs(outer - outer_mix) <= 1 and abs(it - it_mix) <= max(3, it_mix // 10), (it, it_mix, outer, outer_mix)
+    else:  # a slightly different inner operator: a few more corrections are allowed, the answer is the same
+        assert outer <= outer_mix + 3 and it <= 2 * it_mix
     # mismatched contexts are rejected
     import paper_1112_5280_b200 as L
     with pytest.raises(L.LqcdError):

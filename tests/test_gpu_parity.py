@@ -334,3 +334,25 @@ def test_no_writes_outside_the_declared_buffer_sizes(H, precision):
     g.ctx.pack_gauge(gn, torch.from_numpy(np.ascontiguousarray(U)).to("cuda:0"))
     torch.cuda.synchronize()
     assert intact(bp, fb) and intact(bg, g.ctx.gauge_bytes())
+
+
+def test_fp32_spinors_with_half_links(H):
+    """link_precision = 16: fp32 fields, links stored as 12 halfs.  Against the oracle fed the rounded links the
+    result is an ordinary fp32 result (1e-5); against the exact links it is off by the 2^-11 link rounding."""
+    dims, bc = (8, 8, 8, 16), (1, 1, 1, -1)
+    U = li.random_su3_links(dims, seed=97).astype(np.complex64)
+    psi = li.gaussian_spinor(dims, seed=98).astype(np.complex64)
+    g = H.Gpu(dims, 32, 12, bc, U, link_precision=16)
+    assert g.ctx.gauge_bytes() == 2 * 8 * 4096 * 24
+    Uq = _quantise_links(U)
+    for op in (0, 1):
+        got = g.dslash_eo(H.half_of(psi, dims, 1 - op), op)
+        assert H.rel_l2(got, H.half_of(oracle.dslash_eo(Uq, psi, dims, bc, op), dims, op)) <= TOL[32]
+        err = H.rel_l2(got, H.half_of(oracle.dslash_eo(U, psi, dims, bc, op), dims, op))
+        assert 1e-5 < err <= 1e-3
+    refT = H.half_of(oracle.apply_M_tm(Uq, psi, dims, bc, 0.15, 0.3, 1), dims, 0)
+    assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), 0.15, 1, mu=0.3), refT) <= TOL[32]
+    import paper_1112_5280_b200 as L
+    with pytest.raises(L.LqcdError) as e:
+        L.Context(dims, 64, 12, bc, 16)
+    assert e.value.status == L.LQCD_EUNSUPPORTED
