@@ -500,6 +500,13 @@ def run_b200(args):
                                     "us_per_launch": r16["us_per_launch"],
                                     "model": "296 B per site: 2 x (24 halfs + fp32 norm) + 8 x 12 halfs; fp32 arithmetic"}
             del w16
+            w32h = Workload(args.config, 32, 12, dev, args.block, keep_host=False, link_precision=16)
+            r = kernel_leg(torch, dist, w32h, max(1, args.steps // 2), args.warmup, world)
+            nbytes = (48 * 4 + 8 * 24) * w32h.Vh
+            line["fp32_half_links"] = {"gflops": r["gflops"], "us_per_launch": r["us_per_launch"],
+                                       "achieved_gbs": nbytes / (r["us_per_launch"] * 1e-6) / 1e9,
+                                       "model": "384 B per site: fp32 spinors in and out + 8 x 12 halfs"}
+            del w32h
         if rank == 0 and want("cgmixed"):
             w64, w32 = (w2, w) if other == 64 else (w, w2)
             line["cg_fp64"] = cg_leg(torch, w64, tol=1e-10)
