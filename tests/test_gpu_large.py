@@ -140,3 +140,24 @@ def test_config4_properties_at_full_size(cfg4, precision):
     l2 = np.vdot(phi_e.astype(np.complex128), Q(psi_e, mu))
     r2 = np.vdot(Q(phi_e, -mu), psi_e.astype(np.complex128))
     assert abs(l2 - r2) <= tol * abs(l2)
+
+
+def test_largest_lattice_index_headroom():
+    """64^3x128 fp32 recon-12 (V/2 = 16.8 M sites; 12.9 GB of packed links, 9.7 GB canonical): checkerboard
+    indices, tile offsets and byte offsets well past 2^32 bytes; sampled parity against the oracle incl. the corners."""
+    import torch
+    import gpu_harness as H
+    dims, bc = (64, 64, 64, 128), (1, 1, 1, -1)
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40e9:
+        pytest.skip("needs 40 GB of free device memory")
+    U = li.random_su3_links(dims, seed=111, dtype=np.complex64)
+    psi = li.gaussian_spinor(dims, seed=112, dtype=np.complex64)
+    g = H.Gpu(dims, 32, 12, bc, U)
+    assert g.ctx.gauge_bytes() > 2 ** 33
+    for out_parity in (0, 1):
+        got = g.dslash_eo(H.half_of(psi, dims, 1 - out_parity), out_parity)
+        sites = sample_sites(dims, out_parity, 2048, seed=120 + out_parity)
+        ref = oracle.dslash_sites(U, psi, dims, bc, sites)
+        assert H.rel_l2(got[cb_index(dims, sites)], ref) <= TOL[32]
+        assert np.isfinite(got.view(np.float32)).all()
