@@ -169,7 +169,10 @@ template <> struct MinBlocks<float, 18>  { static constexpr int value = LQCD_MIN
 template <> struct MinBlocks<double, 12> { static constexpr int value = LQCD_MINB_F64_R12; };
 template <> struct MinBlocks<double, 18> { static constexpr int value = LQCD_MINB_F64_R18; };
 template <> struct MinBlocks<__half, 12>  { static constexpr int value = LQCD_MINB_F16_R12; };
-template <> struct MinBlocks<float, RECON_12H> { static constexpr int value = LQCD_MINB_F32_R12; };
+#ifndef LQCD_MINB_F32_R12H
+#define LQCD_MINB_F32_R12H 8
+#endif
+template <> struct MinBlocks<float, RECON_12H> { static constexpr int value = LQCD_MINB_F32_R12H; };
 
 // Step K6, the epilogue applied to acc = (H in)(x) before the store (EPI):
 //   EPI_STORE    out = acc                                        lqcd_dslash_*
