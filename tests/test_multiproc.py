@@ -89,3 +89,19 @@ def test_time_slab_ghost_exchange_world2():
         assert g1a == g1b == 16 * other + 1       # right neighbour: its slice 1
         assert own == 16 * r + 1                  # interior untouched
         assert tidx == [(r * Tl - 1 + k) % 16 for k in range(Tl + 2)] and lp == 1
+
+
+def test_reference_arm_prints_the_contract_line():
+    """bench.py --impl reference: one JSON line with the base contract's keys plus impl / cpu_baseline / e2e."""
+    import json
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1", "--warmup", "0",
+                        "--config", "2"], capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-500:]
+    lines = [l for l in r.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "impl", "cpu_baseline", "e2e", "gpu_launches"):
+        assert k in d, k
+    assert d["impl"] == "reference" and d["gpu_launches"] == 0 and d["value"] > 0 and d["vs_baseline"] is None
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
