@@ -185,7 +185,7 @@ class Workload:
         return per_site * self.Vh
 
 
-def timed_steps(torch, dist, fn, steps, warmup):
+def timed_steps(torch, dist, fn, steps, warmup, reduce_device="cuda"):
     """W untimed steps, then K steps between two CUDA events on the launching (current) stream,
     barrier + synchronize on both sides; returns max-over-ranks milliseconds for the K steps."""
     for _ in range(warmup):
@@ -202,7 +202,7 @@ def timed_steps(torch, dist, fn, steps, warmup):
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
-    return max_over_ranks(torch, dist, e0.elapsed_time(e1), "cuda")
+    return max_over_ranks(torch, dist, e0.elapsed_time(e1), reduce_device)
 
 
 def max_over_ranks(torch, dist, ms, device):
@@ -219,11 +219,11 @@ def aggregate_gflops(world, sites_per_step_per_rank, ms_per_step):
     return world * sites_per_step_per_rank * FLOP_PER_SITE / (ms_per_step * 1e-3) / 1e9
 
 
-def kernel_leg(torch, dist, w, steps, warmup, world):
+def kernel_leg(torch, dist, w, steps, warmup, world, reduce_device="cuda"):
     """Device-resident timing of one Workload: returns the numbers of one precision/recon case."""
     L = w.L
     n0 = L.launch_count()
-    ms = timed_steps(torch, dist, w.step, steps, warmup)
+    ms = timed_steps(torch, dist, w.step, steps, warmup, reduce_device)
     launches = (L.launch_count() - n0) - warmup * w.nbuf
     ms_step = ms / steps
     t_launch = ms_step / w.nbuf * 1e-3
@@ -418,13 +418,21 @@ def run_b200(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    # LQCD_BENCH_DEVICE / LQCD_BENCH_BACKEND=gloo: functional test of the N > 1 path on a box with one GPU
+    # (all ranks share the device, host-side barrier and max over ranks through gloo); numbers are then meaningless
+    local = int(os.environ.get("LQCD_BENCH_DEVICE", local))
+    backend = os.environ.get("LQCD_BENCH_BACKEND", "nccl")
+    reduce_device = "cuda" if backend == "nccl" else "cpu"
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     dist = None
     if world > 1:
         import torch.distributed as dist_
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist_.init_process_group("nccl", device_id=dev)
+        if backend == "nccl":
+            dist_.init_process_group("nccl", device_id=dev)
+        else:
+            dist_.init_process_group(backend)
         dist = dist_
     if rank == 0:
         ge.build()
@@ -437,9 +445,9 @@ def run_b200(args):
     w = Workload(args.config, args.precision, args.recon, dev, args.block)
     sampler = ClockSampler(local) if rank == 0 else None
     t0 = time.time()
-    main = kernel_leg(torch, dist, w, args.steps, args.warmup, world)
+    main = kernel_leg(torch, dist, w, args.steps, args.warmup, world, reduce_device)
     # the same region four more times, so the line also shows the spread (value = first region)
-    repeats = [main["ms_per_step"]] + [kernel_leg(torch, dist, w, args.steps, 0, world)["ms_per_step"] for _ in range(4)]
+    repeats = [main["ms_per_step"]] + [kernel_leg(torch, dist, w, args.steps, 0, world, reduce_device)["ms_per_step"] for _ in range(4)]
     # keep the same launches running until nvidia-smi has seen >= 1.5 s of them (clocks under load)
     while time.time() - t0 < 1.5:
         for _ in range(20):
@@ -492,19 +500,19 @@ def run_b200(args):
     if want("other"):
         other = 64 if args.precision == 32 else 32
         w2 = Workload(args.config, other, args.recon, dev, args.block, keep_host=False)
-        r2 = kernel_leg(torch, dist, w2, max(1, args.steps // 2), args.warmup, world)
+        r2 = kernel_leg(torch, dist, w2, max(1, args.steps // 2), args.warmup, world, reduce_device)
         line[f"fp{other}"] = {"gflops": r2["gflops"], "achieved_gbs": r2["gbs"], "frac": r2["gbs"] / peak,
                               "frac_of_nominal_8TBs": r2["gbs"] / NOMINAL_HBM_GBS, "us_per_launch": r2["us_per_launch"],
                               "traffic": ncu_traffic(other, args.recon)}
         if want("fp16") and args.recon == 12:
             w16 = Workload(args.config, 16, 12, dev, args.block, keep_host=False)
-            r16 = kernel_leg(torch, dist, w16, max(1, args.steps // 2), args.warmup, world)
+            r16 = kernel_leg(torch, dist, w16, max(1, args.steps // 2), args.warmup, world, reduce_device)
             line["fp16_storage"] = {"gflops": r16["gflops"], "achieved_gbs": r16["gbs"], "frac": r16["gbs"] / peak,
                                     "us_per_launch": r16["us_per_launch"],
                                     "model": "296 B per site: 2 x (24 halfs + fp32 norm) + 8 x 12 halfs; fp32 arithmetic"}
             del w16
             w32h = Workload(args.config, 32, 12, dev, args.block, keep_host=False, link_precision=16)
-            r = kernel_leg(torch, dist, w32h, max(1, args.steps // 2), args.warmup, world)
+            r = kernel_leg(torch, dist, w32h, max(1, args.steps // 2), args.warmup, world, reduce_device)
             nbytes = (48 * 4 + 8 * 24) * w32h.Vh
             line["fp32_half_links"] = {"gflops": r["gflops"], "us_per_launch": r["us_per_launch"],
                                        "achieved_gbs": nbytes / (r["us_per_launch"] * 1e-6) / 1e9,
