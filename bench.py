@@ -48,7 +48,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=4, help="lattice_inputs.CONFIGS id of the main workload")
-    ap.add_argument("--precision", type=int, default=32, choices=[32, 64], help="precision of the primary line")
+    ap.add_argument("--precision", type=int, default=32, choices=[16, 32, 64], help="precision of the primary line (16: half storage, fp32 arithmetic)")
     ap.add_argument("--recon", type=int, default=12, choices=[12, 18])
     ap.add_argument("--block", type=int, default=0, help="dslash block size override (tuning)")
     ap.add_argument("--chain", action="store_true", help="also time config 5: apply_M(eo=1) x100 chained at 48^3x96")
@@ -461,7 +461,7 @@ def run_b200(args):
     line = {
         "metric": METRIC, "value": main["gflops"], "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": f"f{args.precision}", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32 (f16 storage)" if args.precision == 16 else f"f{args.precision}", "data": "synthetic",
         "config": {
             "workload": f"config {args.config}: {'x'.join(map(str, w.dims))} even-odd dslash, recon-{args.recon}, "
                         f"fp{args.precision}, random SU(3) links seed 1, Gaussian spinors seed 2.., bc (+,+,+,-)",
@@ -483,7 +483,7 @@ def run_b200(args):
             "bound": "hbm", "achieved": main["gbs"], "peak": peak, "unit": "GB/s", "frac": main["gbs"] / peak,
             "traffic": ncu_traffic(args.precision, args.recon), "peak_source": peak_src,
             "kernel": f"dslash_kernel<fp{args.precision}, recon {args.recon}>",
-            "model": f"compulsory {REALS_PER_SITE[args.recon]} reals/site x {args.precision // 8} B x V/2 = {w.bytes_per_launch()} B per launch",
+            "model": f"compulsory bytes, each operand once: {w.bytes_per_launch() // w.Vh} B per site x V/2 = {w.bytes_per_launch()} B per launch",
             "frac_of_nominal_8TBs": main["gbs"] / NOMINAL_HBM_GBS,
         },
     }
@@ -498,7 +498,7 @@ def run_b200(args):
         if want("e2e"):
             line["e2e"] = e2e_leg(torch, w, max(1, min(args.steps, 10)), 1)
     if want("other"):
-        other = 64 if args.precision == 32 else 32
+        other = 32 if args.precision == 64 else 64
         w2 = Workload(args.config, other, args.recon, dev, args.block, keep_host=False)
         r2 = kernel_leg(torch, dist, w2, max(1, args.steps // 2), args.warmup, world, reduce_device)
         line[f"fp{other}"] = {"gflops": r2["gflops"], "achieved_gbs": r2["gbs"], "frac": r2["gbs"] / peak,
