@@ -185,7 +185,11 @@ size_t lqcd_workspace_bytes(const lqcd_ctx* c) { return c ? half_bytes(c) : 0; }
 size_t lqcd_host_workspace_bytes(const lqcd_ctx* c) {
     if (!c) return 0;
     const size_t canon_gauge = (size_t)4 * 2 * c->g.Vh * 18 * canon_elem(c);
-    return align256(lqcd_gauge_bytes(c)) + align256(canon_gauge) + HOST_SLOTS * 4 * align256(half_bytes(c));
+    // per slot: canonical in, native in, native out, canonical out (the canonical half spinor is the larger one
+    // with 16-bit storage)
+    const size_t canon_half = (size_t)24 * c->g.Vh * canon_elem(c);
+    return align256(lqcd_gauge_bytes(c)) + align256(canon_gauge) +
+           HOST_SLOTS * 2 * (align256(half_bytes(c)) + align256(canon_half));
 }
 
 lqcd_status lqcd_set_block_threads(lqcd_ctx* c, int b) {
@@ -548,10 +552,10 @@ lqcd_status lqcd_dslash_eo_host_batch(const lqcd_ctx* c, int n, void* const* out
     char* g_can = base;                 base += align256(canon_gauge);
     char *in_can[HOST_SLOTS], *in_nat[HOST_SLOTS], *out_nat[HOST_SLOTS], *out_can[HOST_SLOTS];
     for (int k = 0; k < HOST_SLOTS; ++k) {
-        in_can[k] = base;  base += align256(hb);
+        in_can[k] = base;  base += align256(cb_bytes);
         in_nat[k] = base;  base += align256(hb);
         out_nat[k] = base; base += align256(hb);
-        out_can[k] = base; base += align256(hb);
+        out_can[k] = base; base += align256(cb_bytes);
     }
     cudaError_t e = cudaSuccess;
     lqcd_status s = LQCD_OK;
