@@ -24,3 +24,13 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _built_library():
+    """Build liblqcd.so (nvcc, sm_100a) and the C oracle once per session if they are missing or stale, so that the
+    tests never depend on a previous build step; the product itself never builds or falls back on its own."""
+    from paper_1112_5280_b200 import _build
+    _build.build()
+    import oracle
+    oracle.build()
