@@ -7,8 +7,10 @@ and achieved HBM GB/s vs roofline at 32^3x64).
 
 Workload (config.workload): BASELINE.json configs[3] = SURVEY.md sec. 8(d) config 4, the headline
 bandwidth case: 32^3x64, even-odd dslash, 12-real links, random SU(3) links (seed 1), Gaussian
-spinors (seed 2), antiperiodic in t.  Primary line fp32; the fp64 case and the config-5 style
-M-chain are reported in the same JSON line under "fp64" and "chain".
+spinors (seed 2), antiperiodic in t.  Primary line fp32.  Further legs ride in the same JSON line (--legs):
+"fp64" (the other precision), "matrix" (apply_M / apply_M_tm), "cg", "cg_fp64", "cg_mixed", "cg_mixed_half_links"
+(the solver), "fp16_storage" and "fp32_half_links" (16-bit storage variants), "e2e" (host buffers), "cpu_baseline"
+(the oracle), and with --chain the config-5 M-chain at 48^3x96.
 
 A step = one pass of the hot path (K1..L6 of SURVEY.md sec. 8(a)) over one batch of NBUF = 4
 half-lattice spinors: NBUF launches of lqcd_dslash_eo, alternating out_parity 0,1 (H_eo, H_oe),
