@@ -473,8 +473,9 @@ def run_b200(args):
                         f"fp{args.precision}, random SU(3) links seed 1, Gaussian spinors seed 2.., bc (+,+,+,-)",
             "step": f"{w.nbuf} lqcd_dslash_eo launches (out_parity 0,1,0,1) over {w.nbuf} distinct in/out half spinors",
             "sites_per_step": w.sites_per_step(),
-            "l2": "inputs larger than L2: links %.0f MB streamed per launch + %.0f MB of rotating spinor buffers; no flush"
-                  % (w.ctx.gauge_bytes() / 1e6, 2 * w.nbuf * w.ctx.spinor_bytes(True) / 1e6),
+            "l2": "inputs larger than L2: links %.0f MB streamed per launch (one parity's half of the packed field) + "
+                  "%.0f MB of rotating spinor buffers; no flush"
+                  % (w.ctx.gauge_bytes() / 2e6, 2 * w.nbuf * w.ctx.spinor_bytes(True) / 1e6),
             "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU",
         },
         "gpu_launches": main["launches"],
