@@ -336,7 +336,9 @@ def matrix_leg(torch, w, napply=50, reps=3):
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / napply
             best = ms if best is None else min(best, ms)
-        nbytes = (2 * REALS_PER_SITE[w.recon] + 24) * (w.precision // 8) * w.Vh
+        nbytes = 2 * w.bytes_per_launch() + w.bytes_per_launch() * 24 // (2 * 24 + 8 * w.recon)  # two passes + the xpay read
+        if w.precision == 16:
+            nbytes = 2 * w.bytes_per_launch() + 52 * w.Vh
         res[name] = {"us_per_application": best * 1e3, "gflops": 2 * FLOP_PER_SITE * w.Vh / (best * 1e-3) / 1e9,
                      "gbs": nbytes / (best * 1e-3) / 1e9}
     return res
