@@ -36,7 +36,7 @@
  *     Sites of one parity are numbered by cb and grouped in tiles of 32 consecutive cb;
  *     ntiles = ceil(V/2 / 32), the last tile is padded (padding is never read or written).
  *     real component r = 6 spin + 2 colour + reim (spinor, 24) or 6 row + 2 col + reim (link,
- *     first `recon` reals of 18).  W = 16 bytes / sizeof(element) reals per 128-bit word.
+ *     first `recon` reals of 18).  W = 32 bytes / sizeof(element) reals per 256-bit spinor word.
  *     half spinor  word q = r / W, lane = r % W  at element ((cb/32 * 24/W + q) * 32 + cb%32) * W + lane
  *     full spinor  [even half | odd half], each of lqcd_spinor_bytes(ctx, 1) bytes
  *     precision 16: a half spinor is 3 16-byte words of 8 halfs per site, [tile][word 3][32], holding v / n(x),
@@ -44,8 +44,8 @@
  *                  of 4 halfs, [parity][tile][hop 8][word 3][32] (52 bytes per spinor site, 24 per link)
  *     links        gathered by output site: [parity p of x][tile][hop k 8][word][32][lane], hop k = 2 mu holds
  *                  U_mu(x), k = 2 mu + 1 holds U_mu(x - mu^) (stored as is; the kernel takes the adjoint).
- *                  Words of 4 floats (recon 12, 3 words), 2 floats (precision 32 recon 18, 9 words of
- *                  8 bytes) or 2 doubles.  Every link is stored twice (capacity for contiguity: all
+ *                  Words of 4 floats (precision 32 recon 12, 3 words), 2 floats (precision 32 recon 18, 9 words),
+ *                  4 doubles (precision 64 recon 12, 3 words) or 2 doubles (precision 64 recon 18, 9 words).  Every link is stored twice (capacity for contiguity: all
  *                  8 links of a warp's 32 sites form one contiguous block); one application of
  *                  lqcd_dslash_eo still reads 8 links per output site exactly once.
  */

@@ -3,10 +3,10 @@
 // Native layout (include/lqcd.h): array of structures of arrays with
 // warp-sized tiles.  Sites of one parity are numbered by their checkerboard index cb and grouped in
 // tiles of TILE = 32 consecutive cb (one warp); ntiles = ceil(Vh / 32), the last tile is padded.
-//   spinor: real r = 6 spin + 2 colour + reim in [0,24); W = 16/sizeof(R) reals per 16-byte word,
+//   spinor: real r = 6 spin + 2 colour + reim in [0,24); W = 32/sizeof(R) reals per 32-byte word,
 //           Q = 24 / W words; word q of site cb at word index ((cb / 32) * Q + q) * 32 + cb % 32.
-//           A warp reads word q of its 32 sites as one 512-byte run, and the Q words of a tile are
-//           adjacent: one contiguous 1.5 KB (fp32) / 3 KB (fp64) block per warp-level gather.
+//           A warp reads word q of its 32 sites as one 1 KB run (one 256-bit access per lane), and the Q
+//           words of a tile are adjacent: one contiguous 3 KB (fp32) / 6 KB (fp64) block per warp-level gather.
 //   links:  "gathered by output site": for the site cb of parity p, hop k = 2 mu + (backward ? 1 : 0)
 //           holds U_mu(x) (k even) or U_mu(x - mu^) (k odd), first RECON reals r = 6 row + 2 col + reim,
 //           in words of LW reals; word w at ((((p * ntiles + cb / 32) * 8 + k) * NW + w) * 32 + cb % 32.
@@ -24,19 +24,53 @@ constexpr int TILE = 32;
 __device__ __forceinline__ float fmar(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ double fmar(double a, double b, double c) { return fma(a, b, c); }
 
-template <typename R> struct Word;            // 128-bit word of R
-template <> struct Word<float>  { using type = float4;  static constexpr int W = 4; };
-template <> struct Word<double> { using type = double2; static constexpr int W = 2; };
+// Spinor word: 32 bytes, read and written with Blackwell's 256-bit global accesses (LDG.256 / STG.256,
+// ld.global.v8.f32 / .v4.f64 on sm_100): half as many memory instructions per byte as 128-bit words.
+struct __align__(32) float8_ { float v[8]; };
+struct __align__(32) double4_ { double v[4]; };
+template <typename R> struct Word;
+template <> struct Word<float>  { using type = float8_;  static constexpr int W = 8; };
+template <> struct Word<double> { using type = double4_; static constexpr int W = 4; };
 
-// Link word: 16 bytes except fp32 18-real (18 = 4.5 x 4, so 9 x float2).
-template <typename R, int RECON> struct LinkWord { using type = typename Word<R>::type; static constexpr int LW = Word<R>::W; };
-template <> struct LinkWord<float, 18> { using type = float2; static constexpr int LW = 2; };
+// Link word: the largest of 32 / 16 / 8 bytes that divides the stored reals (fp32 12-real: 3 x 16 B; fp32 18-real:
+// 9 x 8 B; fp64 12-real: 3 x 32 B; fp64 18-real: 9 x 16 B).
+template <typename R, int RECON> struct LinkWord;
+template <> struct LinkWord<float, 12>  { using type = float4;   static constexpr int LW = 4; };
+template <> struct LinkWord<float, 18>  { using type = float2;   static constexpr int LW = 2; };
+template <> struct LinkWord<double, 12> { using type = double4_; static constexpr int LW = 4; };
+template <> struct LinkWord<double, 18> { using type = double2;  static constexpr int LW = 2; };
+template <> struct LinkWord<float, 13>  { using type = float4;   static constexpr int LW = 4; };  // RECON_12H: unused (half links)
 
 __device__ __forceinline__ void unpack(const float4& w, float* v)  { v[0] = w.x; v[1] = w.y; v[2] = w.z; v[3] = w.w; }
 __device__ __forceinline__ void unpack(const float2& w, float* v)  { v[0] = w.x; v[1] = w.y; }
 __device__ __forceinline__ void unpack(const double2& w, double* v) { v[0] = w.x; v[1] = w.y; }
-__device__ __forceinline__ float4  pack4(const float* v)  { return make_float4(v[0], v[1], v[2], v[3]); }
-__device__ __forceinline__ double2 pack2(const double* v) { return make_double2(v[0], v[1]); }
+__device__ __forceinline__ void unpack(const float8_& w, float* v) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = w.v[i];
+}
+__device__ __forceinline__ void unpack(const double4_& w, double* v) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) v[i] = w.v[i];
+}
+
+__device__ __forceinline__ float8_ ldg256(const float8_* p) {
+    float8_ w;
+    asm("ld.global.nc.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+        : "=f"(w.v[0]), "=f"(w.v[1]), "=f"(w.v[2]), "=f"(w.v[3]), "=f"(w.v[4]), "=f"(w.v[5]), "=f"(w.v[6]), "=f"(w.v[7]) : "l"(p));
+    return w;
+}
+__device__ __forceinline__ double4_ ldg256(const double4_* p) {
+    double4_ w;
+    asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(w.v[0]), "=d"(w.v[1]), "=d"(w.v[2]), "=d"(w.v[3]) : "l"(p));
+    return w;
+}
+__device__ __forceinline__ void stg256(float8_* p, const float* v) {
+    asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]),
+                 "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
+}
+__device__ __forceinline__ void stg256(double4_* p, const double* v) {
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v[0]), "d"(v[1]), "d"(v[2]), "d"(v[3]) : "memory");
+}
 
 // word 0 of site cb in a native half spinor; word q is q * TILE words further on
 template <typename R>
@@ -61,7 +95,7 @@ __device__ __forceinline__ void load_spinor(const R* __restrict__ base, int cb, 
     const Wd* p = reinterpret_cast<const Wd*>(base) + spinor_word0<R>(cb);
 #pragma unroll
     for (int q = 0; q < Q; ++q) {
-        Wd w = __ldg(p + q * TILE);
+        Wd w = ldg256(p + q * TILE);
         unpack(w, v + q * W);
     }
 }
@@ -72,11 +106,7 @@ __device__ __forceinline__ void store_spinor(R* __restrict__ base, int cb, const
     constexpr int W = Word<R>::W, Q = 24 / W;
     Wd* p = reinterpret_cast<Wd*>(base) + spinor_word0<R>(cb);
 #pragma unroll
-    for (int q = 0; q < Q; ++q) {
-        Wd w;
-        if constexpr (W == 4) w = pack4(v + q * W); else w = pack2(v + q * W);
-        p[q * TILE] = w;
-    }
+    for (int q = 0; q < Q; ++q) stg256(p + q * TILE, v + q * W);
 }
 
 // Links are read exactly once per application: streaming loads (ld.global.cs, evict-first)
@@ -84,6 +114,7 @@ __device__ __forceinline__ void store_spinor(R* __restrict__ base, int cb, const
 __device__ __forceinline__ float4  ld_stream(const float4* p)  { return __ldcs(p); }
 __device__ __forceinline__ float2  ld_stream(const float2* p)  { return __ldcs(p); }
 __device__ __forceinline__ double2 ld_stream(const double2* p) { return __ldcs(p); }
+__device__ __forceinline__ double4_ ld_stream(const double4_* p) { return ldg256(p); }  // 256-bit: no .cs form; policy is immaterial here
 
 // K2: rebuild row 2 of u[18] (row-major 3x3 complex, u[6 row + 2 col + reim]) as conj(row0 x row1);
 // valid for det U = +1 ("RECONSTRUCT TWELVE").
