@@ -22,7 +22,9 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
  *     entry points only enqueue work and return; they never synchronise.  The *_host entry points
  *     and the CG solvers synchronise `stream` before returning (their results live in host memory).
- *   - All device field pointers must be 16-byte aligned (LQCD_EALIGN otherwise).
+ *   - Native device fields (spinors, links, workspaces) are accessed with 256-bit words and must be 32-byte
+ *     aligned for every precision; canonical device buffers 16-byte aligned; the solver and host-path
+ *     workspaces 256-byte aligned.  A misaligned pointer returns LQCD_EALIGN before anything is launched.
  *   - The stencil is not in-place safe: `out` overlapping `in` / `workspace` gives LQCD_EALIAS.
  *   - Errors are return codes only: nothing throws, aborts or prints.
  *
@@ -63,7 +65,7 @@ typedef struct lqcd_ctx lqcd_ctx; /* opaque: geometry + constants, host memory *
 typedef enum {
     LQCD_OK = 0,
     LQCD_EINVAL = 1,       /* null pointer, bad extent / parity / precision / recon, |bc| != 1 */
-    LQCD_EALIGN = 2,       /* a device pointer is not 16-byte aligned */
+    LQCD_EALIGN = 2,       /* a device pointer is misaligned: native 32 B, canonical 16 B, big workspaces 256 B */
     LQCD_EALIAS = 3,       /* out overlaps in or workspace */
     LQCD_EUNSUPPORTED = 4, /* combination not compiled in */
     LQCD_ECUDA = 5         /* CUDA runtime / launch error */
@@ -202,10 +204,6 @@ lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* ctx, void* out_host, const void*
 
 /* Number of kernels this library has launched since load (a claim counter for bench.py). */
 unsigned long long lqcd_launch_count(void);
-
-/* Launch-geometry knobs for tuning runs; 0 restores the default.  Returns LQCD_EINVAL if the
- * value is not supported.  block_threads in {64,128}. */
-lqcd_status lqcd_set_block_threads(lqcd_ctx* ctx, int block_threads);
 
 const char* lqcd_status_string(lqcd_status s);
 const char* lqcd_last_cuda_error(void); /* text of the last CUDA error seen by this thread's calls */

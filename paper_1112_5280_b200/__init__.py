@@ -19,7 +19,7 @@ EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
     "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_set_time_slab", "lqcd_dslash_eo_range", "lqcd_time_slice_bytes", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_dslash_eo_host_batch", "lqcd_launch_count",
-    "lqcd_set_block_threads", "lqcd_status_string", "lqcd_last_cuda_error",
+    "lqcd_status_string", "lqcd_last_cuda_error",
 ]
 
 
@@ -77,7 +77,6 @@ def _lib():
         lib.lqcd_dslash_eo_host_batch.argtypes = [vp, ci, ctypes.POINTER(vp), vp, ctypes.POINTER(vp), ctypes.POINTER(ci), vp, vp]
         lib.lqcd_launch_count.argtypes = []
         lib.lqcd_launch_count.restype = ctypes.c_ulonglong
-        lib.lqcd_set_block_threads.argtypes = [vp, ci]
         lib.lqcd_status_string.argtypes = [ci]
         lib.lqcd_status_string.restype = ctypes.c_char_p
         lib.lqcd_last_cuda_error.argtypes = []
@@ -135,9 +134,6 @@ class Context:
     def workspace_bytes(self): return _lib().lqcd_workspace_bytes(self._h)
     def host_workspace_bytes(self): return _lib().lqcd_host_workspace_bytes(self._h)
     def cg_workspace_bytes(self): return _lib().lqcd_cg_workspace_bytes(self._h)
-
-    def set_block_threads(self, n):
-        _chk(_lib().lqcd_set_block_threads(self._h, int(n)), "lqcd_set_block_threads")
 
     # layout conversion
     def pack_gauge(self, native, canonical, stream=None):

@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_scalar_kernel(const double* __r
 
 // x += alpha p;  r -= alpha s;  partial = block sums of |r|^2       (skipped once done)
 template <typename R>
-__global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(R* __restrict__ x, R* __restrict__ r, const R* __restrict__ p,
+__global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(R* x, R* r, const R* __restrict__ p,
                                                                    const R* __restrict__ s, Geom g, const CgScalars* __restrict__ sc,
                                                                    double* __restrict__ partial) {
     const int cb = blockIdx.x * BLAS_BLOCK + threadIdx.x;
@@ -94,10 +94,10 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(R* __restrict_
     double n2 = 0.0;
     if (cb < g.Vh) {
         R rv[24];
-        load_spinor<R>(r, cb, rv);
+        load_spinor_rw<R>(r, cb, rv);   // r and x are updated in place: coherent loads, not .nc
         if (!done) {
             R xv[24], pv[24], sv[24];
-            load_spinor<R>(x, cb, xv);
+            load_spinor_rw<R>(x, cb, xv);
             load_spinor<R>(p, cb, pv);
             load_spinor<R>(s, cb, sv);
 #pragma unroll
@@ -116,13 +116,13 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(R* __restrict_
 
 // p = r + beta p       (skipped once done)
 template <typename R>
-__global__ void __launch_bounds__(BLAS_BLOCK) cg_update_p_kernel(R* __restrict__ p, const R* __restrict__ r, Geom g,
+__global__ void __launch_bounds__(BLAS_BLOCK) cg_update_p_kernel(R* p, const R* __restrict__ r, Geom g,
                                                                   const CgScalars* __restrict__ sc) {
     const int cb = blockIdx.x * BLAS_BLOCK + threadIdx.x;
     if (cb >= g.Vh || sc->done) return;
     const R beta = (R)sc->beta;
     R pv[24], rv[24];
-    load_spinor<R>(p, cb, pv);
+    load_spinor_rw<R>(p, cb, pv);   // p is updated in place
     load_spinor<R>(r, cb, rv);
 #pragma unroll
     for (int k = 0; k < 24; ++k) pv[k] = fmar(beta, pv[k], rv[k]);
@@ -145,12 +145,12 @@ __global__ void __launch_bounds__(BLAS_BLOCK) convert_kernel(Rd* __restrict__ ds
 }
 
 // x += (double) e
-__global__ void __launch_bounds__(BLAS_BLOCK) accumulate_correction_kernel(double* __restrict__ x, const float* __restrict__ e, Geom g) {
+__global__ void __launch_bounds__(BLAS_BLOCK) accumulate_correction_kernel(double* x, const float* __restrict__ e, Geom g) {
     const int cb = blockIdx.x * BLAS_BLOCK + threadIdx.x;
     if (cb >= g.Vh) return;
     double xv[24];
     float ev[24];
-    load_spinor<double>(x, cb, xv);
+    load_spinor_rw<double>(x, cb, xv);   // x is updated in place
     load_spinor<float>(e, cb, ev);
 #pragma unroll
     for (int k = 0; k < 24; ++k) xv[k] += (double)ev[k];

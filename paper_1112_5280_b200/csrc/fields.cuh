@@ -1,4 +1,4 @@
-// fields.cuh -- native field layout (step L0) and 128-bit loads/stores (L1, L2, L6), K2 recon.
+// fields.cuh -- native field layout (step L0), 256-/128-bit loads and stores (L1, L2, L6), K2 recon.
 //
 // Native layout (include/lqcd.h): array of structures of arrays with
 // warp-sized tiles.  Sites of one parity are numbered by their checkerboard index cb and grouped in
@@ -64,6 +64,20 @@ __device__ __forceinline__ double4_ ldg256(const double4_* p) {
     asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(w.v[0]), "=d"(w.v[1]), "=d"(w.v[2]), "=d"(w.v[3]) : "l"(p));
     return w;
 }
+// Plain (coherent) 256-bit loads for operands the same kernel overwrites (the in-place BLAS-1 updates): .nc is only
+// legal for locations that stay read-only for the whole kernel.
+__device__ __forceinline__ float8_ ld256(const float8_* p) {
+    float8_ w;
+    asm volatile("ld.global.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=f"(w.v[0]), "=f"(w.v[1]), "=f"(w.v[2]), "=f"(w.v[3]), "=f"(w.v[4]), "=f"(w.v[5]), "=f"(w.v[6]), "=f"(w.v[7])
+                 : "l"(p) : "memory");
+    return w;
+}
+__device__ __forceinline__ double4_ ld256(const double4_* p) {
+    double4_ w;
+    asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(w.v[0]), "=d"(w.v[1]), "=d"(w.v[2]), "=d"(w.v[3]) : "l"(p) : "memory");
+    return w;
+}
 __device__ __forceinline__ void stg256(float8_* p, const float* v) {
     asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]),
                  "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
@@ -86,8 +100,8 @@ __host__ __device__ __forceinline__ size_t link_word0(int ntiles, int p, int cb,
     return ((size_t)(p * ntiles + cb / TILE) * 8 + k) * (NW * TILE) + (cb % TILE);
 }
 
-// Spinor loads take the default cached path: each input spinor is gathered by 8 output
-// sites, and that reuse must come from L1/L2, not from DRAM.
+// Spinor loads go through the read-only path (ld.global.nc) with default caching: each input spinor is gathered
+// by 8 output sites, and that reuse must come from L1/L2, not from DRAM.  Only for fields the kernel never writes.
 template <typename R>
 __device__ __forceinline__ void load_spinor(const R* __restrict__ base, int cb, R v[24]) {
     using Wd = typename Word<R>::type;
@@ -96,6 +110,19 @@ __device__ __forceinline__ void load_spinor(const R* __restrict__ base, int cb, 
 #pragma unroll
     for (int q = 0; q < Q; ++q) {
         Wd w = ldg256(p + q * TILE);
+        unpack(w, v + q * W);
+    }
+}
+
+// the same for a field the calling kernel also writes (x, r, p of the CG updates): coherent loads
+template <typename R>
+__device__ __forceinline__ void load_spinor_rw(const R* base, int cb, R v[24]) {
+    using Wd = typename Word<R>::type;
+    constexpr int W = Word<R>::W, Q = 24 / W;
+    const Wd* p = reinterpret_cast<const Wd*>(base) + spinor_word0<R>(cb);
+#pragma unroll
+    for (int q = 0; q < Q; ++q) {
+        Wd w = ld256(p + q * TILE);
         unpack(w, v + q * W);
     }
 }

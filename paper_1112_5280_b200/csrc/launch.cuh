@@ -1,0 +1,78 @@
+// launch.cuh -- host-side launch chain of the dslash kernel, shared by lqcd.cu (which only calls it) and the
+// instantiation units inst_*.cu (one per storage type x link format, so that the library builds in parallel:
+// each unit instantiates dslash_kernel for its 4 epilogues x 2 boundary-phase kinds).
+#pragma once
+#include "../../include/lqcd.h"
+
+#include "dslash_kernel.cuh"
+
+struct lqcd_ctx {
+    lqcd_params p;
+    lqcd::Geom g;
+    bool complex_bc;
+};
+
+namespace lqcd {
+
+// threads per block of the dslash kernel: 64 (two warp tiles).  128 measured the same on B200.
+#ifndef LQCD_BLOCK
+#define LQCD_BLOCK 64
+#endif
+constexpr int DSLASH_BLOCK = LQCD_BLOCK;
+
+// counts the launch and picks up a launch error (defined in lqcd.cu)
+lqcd_status after_launch();
+
+// epilogue of one launch: mode (EPI_*) and its constants, in double until the kernel's precision is known
+struct EpiArgs { int mode; double a, g_re, g_im; int g5_out; };
+
+// range of checkerboard indices one launch covers: everything, or the time slices [t_begin, t_end)
+struct CbRange { int begin, end; };
+
+template <typename R>
+BcPhases<R> make_bc(const lqcd_ctx* c) {
+    BcPhases<R> b;
+    for (int mu = 0; mu < 4; ++mu) {
+        b.re[mu] = (R)c->p.bc_re[mu];
+        b.im[mu] = (R)c->p.bc_im[mu];
+    }
+    return b;
+}
+
+template <typename S, int RECON, int EPI, bool CBC>
+lqcd_status launch_one(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                       const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
+    constexpr int BLOCK = DSLASH_BLOCK;
+    const dim3 grid((rg.end - rg.begin + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
+    using A = typename Compute<S>::type;  // S is the storage type, A the arithmetic type
+    const Epilogue<A> epi{(A)e.a, (A)e.g_re, (A)e.g_im, e.g5_out};
+    dslash_kernel<S, RECON, EPI, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
+        (S*)out, (const S*)gauge, (const S*)in, (const S*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<A>(c), rg.begin, rg.end);
+    return after_launch();
+}
+
+template <typename S, int RECON, int EPI>
+lqcd_status launch_epi(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                       const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
+    return c->complex_bc ? launch_one<S, RECON, EPI, true>(c, out, gauge, in, xin, e, parity, st, rg)
+                         : launch_one<S, RECON, EPI, false>(c, out, gauge, in, xin, e, parity, st, rg);
+}
+
+// out_p = epilogue(H in) for one storage type and link format; parity < 0: both parities, full fields.
+// Explicitly instantiated in inst_*.cu.
+template <typename S, int RECON>
+lqcd_status launch_recon(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                         const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
+    switch (e.mode) {
+        case EPI_STORE: return launch_epi<S, RECON, EPI_STORE>(c, out, gauge, in, xin, e, parity, st, rg);
+        case EPI_XPAY: return launch_epi<S, RECON, EPI_XPAY>(c, out, gauge, in, xin, e, parity, st, rg);
+        case EPI_G5SCALE: return launch_epi<S, RECON, EPI_G5SCALE>(c, out, gauge, in, xin, e, parity, st, rg);
+        case EPI_G5XPAY: return launch_epi<S, RECON, EPI_G5XPAY>(c, out, gauge, in, xin, e, parity, st, rg);
+    }
+    return LQCD_EUNSUPPORTED;
+}
+
+#define LQCD_LAUNCH_RECON_ARGS \
+    const lqcd_ctx*, void*, const void*, const void*, const void*, const EpiArgs&, int, cudaStream_t, CbRange
+
+}  // namespace lqcd

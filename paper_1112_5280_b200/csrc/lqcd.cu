@@ -2,8 +2,6 @@
 // dispatch (storage precision x recon x epilogue x bc kind x block size), kernel launches, the CG
 // loops and the pipelined host-buffer path.  No field memory is allocated here; only the entry points
 // that return results to host memory (lqcd_dslash_eo_host*, lqcd_cg_solve_tm*) synchronise.
-#include "../../include/lqcd.h"
-
 #include <atomic>
 #include <cmath>
 #include <cstdint>
@@ -11,17 +9,20 @@
 #include <new>
 
 #include "blas_kernels.cuh"
-#include "dslash_kernel.cuh"
+#include "launch.cuh"
 #include "pack_kernels.cuh"
 
 using namespace lqcd;
 
-struct lqcd_ctx {
-    lqcd_params p;
-    Geom g;
-    bool complex_bc;
-    int block;    // threads per block of the dslash kernel
-};
+namespace lqcd {
+// the dslash kernels are instantiated in inst_*.cu
+extern template lqcd_status launch_recon<double, 12>(LQCD_LAUNCH_RECON_ARGS);
+extern template lqcd_status launch_recon<double, 18>(LQCD_LAUNCH_RECON_ARGS);
+extern template lqcd_status launch_recon<float, 12>(LQCD_LAUNCH_RECON_ARGS);
+extern template lqcd_status launch_recon<float, 18>(LQCD_LAUNCH_RECON_ARGS);
+extern template lqcd_status launch_recon<__half, 12>(LQCD_LAUNCH_RECON_ARGS);
+extern template lqcd_status launch_recon<float, RECON_12H>(LQCD_LAUNCH_RECON_ARGS);
+}  // namespace lqcd
 
 namespace {
 
@@ -33,12 +34,19 @@ lqcd_status cuda_fail(cudaError_t e) {
     return LQCD_ECUDA;
 }
 
-lqcd_status after_launch() {
+}  // namespace
+
+lqcd_status lqcd::after_launch() {
     g_launches.fetch_add(1, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? LQCD_OK : cuda_fail(e);
 }
 
+namespace {
+
+// Native fields are read and written with 256-bit words (fields.cuh): 32-byte alignment.  Canonical
+// (interchange) buffers are only touched element by element by the pack kernels: the natural 16 bytes of a complex128.
+inline bool aligned32(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 31u) == 0; }
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 inline bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
@@ -55,62 +63,7 @@ inline size_t half_bytes(const lqcd_ctx* c) {
 inline size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
 constexpr int HOST_SLOTS = 3;  // pipeline depth of lqcd_dslash_eo_host_batch
 
-template <typename R>
-BcPhases<R> make_bc(const lqcd_ctx* c) {
-    BcPhases<R> b;
-    for (int mu = 0; mu < 4; ++mu) {
-        b.re[mu] = (R)c->p.bc_re[mu];
-        b.im[mu] = (R)c->p.bc_im[mu];
-    }
-    return b;
-}
-
-// epilogue of one launch: mode (EPI_*) and its constants, in double until the kernel's precision is known
-struct EpiArgs { int mode; double a, g_re, g_im; int g5_out; };
-
-// range of checkerboard indices one launch covers: everything, or the time slices [t_begin, t_end)
-struct CbRange { int begin, end; };
 inline CbRange all_sites(const lqcd_ctx* c) { return CbRange{0, c->g.Vh}; }
-
-template <typename R, int RECON, int EPI, bool CBC, int BLOCK>
-lqcd_status launch_block(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                         const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
-    const dim3 grid((rg.end - rg.begin + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
-    using A = typename Compute<R>::type;  // R is the storage type here, A the arithmetic type
-    const Epilogue<A> epi{(A)e.a, (A)e.g_re, (A)e.g_im, e.g5_out};
-    dslash_kernel<R, RECON, EPI, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
-        (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<A>(c), rg.begin, rg.end);
-    return after_launch();
-}
-
-template <typename R, int RECON, int EPI, bool CBC>
-lqcd_status launch_cbc(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                       const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
-    switch (c->block) {
-        case 64: return launch_block<R, RECON, EPI, CBC, 64>(c, out, gauge, in, xin, e, parity, st, rg);
-        case 128: return launch_block<R, RECON, EPI, CBC, 128>(c, out, gauge, in, xin, e, parity, st, rg);
-    }
-    return LQCD_EUNSUPPORTED;
-}
-
-template <typename R, int RECON, int EPI>
-lqcd_status launch_epi(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                       const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
-    return c->complex_bc ? launch_cbc<R, RECON, EPI, true>(c, out, gauge, in, xin, e, parity, st, rg)
-                         : launch_cbc<R, RECON, EPI, false>(c, out, gauge, in, xin, e, parity, st, rg);
-}
-
-template <typename R, int RECON>
-lqcd_status launch_recon(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
-                         const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
-    switch (e.mode) {
-        case EPI_STORE: return launch_epi<R, RECON, EPI_STORE>(c, out, gauge, in, xin, e, parity, st, rg);
-        case EPI_XPAY: return launch_epi<R, RECON, EPI_XPAY>(c, out, gauge, in, xin, e, parity, st, rg);
-        case EPI_G5SCALE: return launch_epi<R, RECON, EPI_G5SCALE>(c, out, gauge, in, xin, e, parity, st, rg);
-        case EPI_G5XPAY: return launch_epi<R, RECON, EPI_G5XPAY>(c, out, gauge, in, xin, e, parity, st, rg);
-    }
-    return LQCD_EUNSUPPORTED;
-}
 
 // out_p = epilogue(H in); parity < 0: both parities, full fields.
 lqcd_status launch_dslash(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
@@ -127,7 +80,7 @@ lqcd_status launch_dslash(const lqcd_ctx* c, void* out, const void* gauge, const
 
 lqcd_status check_fields(const lqcd_ctx* c, const void* out, const void* gauge, const void* in, size_t nbytes) {
     if (!c || !out || !gauge || !in) return LQCD_EINVAL;
-    if (!aligned16(out) || !aligned16(gauge) || !aligned16(in)) return LQCD_EALIGN;
+    if (!aligned32(out) || !aligned32(gauge) || !aligned32(in)) return LQCD_EALIGN;
     if (overlaps(out, nbytes, in, nbytes)) return LQCD_EALIAS;
     return LQCD_OK;
 }
@@ -165,7 +118,6 @@ lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p) {
     g.sy = g.Xh; g.sz = g.Xh * g.Y; g.st = g.Xh * g.Y * g.Z;
     g.tcf = g.T - 1; g.tcb = 0;
     c->complex_bc = cbc;
-    c->block = 64;
     *ctx = c;
     return LQCD_OK;
 }
@@ -192,17 +144,9 @@ size_t lqcd_host_workspace_bytes(const lqcd_ctx* c) {
            HOST_SLOTS * 2 * (align256(half_bytes(c)) + align256(canon_half));
 }
 
-lqcd_status lqcd_set_block_threads(lqcd_ctx* c, int b) {
-    if (!c) return LQCD_EINVAL;
-    if (b == 0) b = 64;
-    if (b != 64 && b != 128) return LQCD_EINVAL;
-    c->block = b;
-    return LQCD_OK;
-}
-
 lqcd_status lqcd_pack_gauge(const lqcd_ctx* c, void* native, const void* canon, void* stream) {
     if (!c || !native || !canon) return LQCD_EINVAL;
-    if (!aligned16(native) || !aligned16(canon)) return LQCD_EALIGN;
+    if (!aligned32(native) || !aligned16(canon)) return LQCD_EALIGN;
     const dim3 grid((c->g.Vh + 127) / 128, 8, 2);
     cudaStream_t st = (cudaStream_t)stream;
     if (c->p.precision == 16 || c->p.link_precision == 16) {
@@ -220,7 +164,7 @@ lqcd_status lqcd_pack_gauge(const lqcd_ctx* c, void* native, const void* canon, 
 static lqcd_status pack_unpack(const lqcd_ctx* c, void* dst, const void* src, int parity, void* stream, bool unpack) {
     if (!c || !dst || !src) return LQCD_EINVAL;
     if (parity < -1 || parity > 1) return LQCD_EINVAL;
-    if (!aligned16(dst) || !aligned16(src)) return LQCD_EALIGN;
+    if (!aligned32(unpack ? src : dst) || !aligned16(unpack ? dst : src)) return LQCD_EALIGN;  // native 32, canonical 16
     const dim3 grid((c->g.Vh + 127) / 128, parity < 0 ? 2 : 1);
     cudaStream_t st = (cudaStream_t)stream;
     if (c->p.precision == 16) {
@@ -303,7 +247,7 @@ static lqcd_status apply_M_impl(const lqcd_ctx* c, void* out, const void* gauge,
     lqcd_status s = check_fields(c, out, gauge, in, hb);
     if (s != LQCD_OK) return s;
     if (!workspace) return LQCD_EINVAL;
-    if (!aligned16(workspace)) return LQCD_EALIGN;
+    if (!aligned32(workspace)) return LQCD_EALIGN;
     if (overlaps(workspace, hb, in, hb) || overlaps(workspace, hb, out, hb)) return LQCD_EALIAS;
     // tmp_o = (1 + i theta g5)^-1 H_oe in_e, with (1 + i theta g5)^-1 = (1 - i theta g5) / (1 + theta^2)
     const double n = 1.0 / (1.0 + theta * theta);
@@ -475,7 +419,7 @@ lqcd_status lqcd_cg_solve_tm_mixed(const lqcd_ctx* c64, const lqcd_ctx* c32, voi
     lqcd_status s = check_fields(c64, x, gauge64, b, hb64);
     if (s != LQCD_OK) return s;
     if (!workspace || !(tol > 0.0) || !(inner_tol > 0.0) || maxiter < 0) return LQCD_EINVAL;
-    if (!aligned16(gauge32)) return LQCD_EALIGN;
+    if (!aligned32(gauge32)) return LQCD_EALIGN;
     if (reinterpret_cast<uintptr_t>(workspace) & 255u) return LQCD_EALIGN;
     const size_t wb = lqcd_cg_mixed_workspace_bytes(c64, c32);
     if (overlaps(workspace, wb, x, hb64) || overlaps(workspace, wb, b, hb64)) return LQCD_EALIAS;
@@ -628,7 +572,7 @@ const char* lqcd_status_string(lqcd_status s) {
     switch (s) {
         case LQCD_OK: return "ok";
         case LQCD_EINVAL: return "invalid argument";
-        case LQCD_EALIGN: return "device pointer not 16-byte aligned";
+        case LQCD_EALIGN: return "device pointer not aligned (native fields: 32 bytes, canonical buffers: 16, solver / host workspaces: 256)";
         case LQCD_EALIAS: return "output overlaps an input";
         case LQCD_EUNSUPPORTED: return "unsupported configuration";
         case LQCD_ECUDA: return "CUDA error";

@@ -53,9 +53,6 @@ def test_create_validation_and_sizes():
         with pytest.raises(L.LqcdError) as e:
             L.Context(**kw)
         assert e.value.status == L.LQCD_EINVAL
-    c.set_block_threads(128)
-    with pytest.raises(L.LqcdError):
-        c.set_block_threads(100)
 
 
 def test_null_pointers_rejected_without_gpu():
@@ -66,3 +63,26 @@ def test_null_pointers_rejected_without_gpu():
     assert lib.lqcd_apply_M(c._h, None, None, None, 0.1, 2, None, None) == L.LQCD_EINVAL
     assert lib.lqcd_spinor_bytes(None, 1) == 0
     assert lib.lqcd_status_string(L.LQCD_EALIAS).decode() == "output overlaps an input"
+
+
+def test_alignment_contract_checked_before_any_launch():
+    """Native fields are accessed with 256-bit words: every native pointer must be 32-byte aligned, canonical buffers
+    16-byte aligned.  The check precedes any CUDA call, so fake addresses exercise it without a GPU."""
+    lib = L._lib()
+    base = 1 << 20
+    for precision, recon in ((64, 12), (64, 18), (32, 12), (32, 18), (16, 12)):
+        c = L.Context((4, 4, 4, 4), precision, recon)
+        far = base + (1 << 16)
+        for off in (8, 16, 24):
+            assert lib.lqcd_dslash_eo(c._h, base + off, base + (1 << 18), far, 0, None) == L.LQCD_EALIGN
+            assert lib.lqcd_dslash_eo(c._h, base, base + (1 << 18) + off, far, 0, None) == L.LQCD_EALIGN
+            assert lib.lqcd_dslash_eo(c._h, base, base + (1 << 18), far + off, 0, None) == L.LQCD_EALIGN
+            assert lib.lqcd_dslash_full(c._h, base + off, base + (1 << 18), far + (1 << 16), None) == L.LQCD_EALIGN
+            assert lib.lqcd_apply_M(c._h, base, base + (1 << 18), far, 0.1, 1, base + (1 << 17) + off, None) == L.LQCD_EALIGN
+            assert lib.lqcd_apply_M(c._h, base + off, base + (1 << 18), far, 0.1, 0, None, None) == L.LQCD_EALIGN
+            assert lib.lqcd_pack_spinor(c._h, base + off, far, 0, None) == L.LQCD_EALIGN      # native side: 32
+            assert lib.lqcd_unpack_spinor(c._h, far, base + off, 0, None) == L.LQCD_EALIGN
+            assert lib.lqcd_pack_gauge(c._h, base + off, far, None) == L.LQCD_EALIGN
+        assert lib.lqcd_pack_spinor(c._h, base, far + 8, 0, None) == L.LQCD_EALIGN            # canonical side: 16
+        assert lib.lqcd_unpack_spinor(c._h, far + 8, base, 0, None) == L.LQCD_EALIGN
+    assert b"32" in lib.lqcd_status_string(L.LQCD_EALIGN)

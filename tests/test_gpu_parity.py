@@ -35,9 +35,9 @@ def test_config1_full_fp64(H, recon):
     c, U, psi = _inputs(1, 64)
     g = H.Gpu(c["dims"], 64, recon, c["bc"], U)
     ref = oracle.dslash_full(U, psi, c["dims"], c["bc"])
-    assert H.rel_l2(g.dslash_full(psi), ref) <= TOL[64]
+    H.assert_parity(g.dslash_full(psi), ref, 64)
     refM = oracle.apply_M(U, psi, c["dims"], c["bc"], c["kappa"], 0)
-    assert H.rel_l2(g.apply_M(psi, c["kappa"], 0), refM) <= TOL[64]
+    H.assert_parity(g.apply_M(psi, c["kappa"], 0), refM, 64)
 
 
 def test_config1_free_field_plane_wave(H):
@@ -54,7 +54,7 @@ def test_config1_free_field_plane_wave(H):
         for mu in range(4):
             m = m + 2j * kappa * np.sin(p[mu]) * oracle.gamma(mu)
         expect = np.einsum("st,...ta->...sa", m, psi)
-        assert H.rel_l2(g.apply_M(psi, kappa, 0), expect) <= TOL[64]
+        H.assert_parity(g.apply_M(psi, kappa, 0), expect, 64)
 
 
 # ------------------------------------------------------------------ config 2: 8^3x16 fp64 eo
@@ -66,12 +66,12 @@ def test_config2_eo_fp64(H, recon):
     for out_parity in (0, 1):
         ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, out_parity), dims, out_parity)
         got = g.dslash_eo(H.half_of(psi, dims, 1 - out_parity), out_parity)
-        assert H.rel_l2(got, ref) <= TOL[64]
+        H.assert_parity(got, ref, 64)
     # even-odd pieces reassemble the full operator (pin P4 on the GPU)
     full = g.dslash_full(psi)
-    assert H.rel_l2(full, oracle.dslash_full(U, psi, dims, bc)) <= TOL[64]
+    H.assert_parity(full, oracle.dslash_full(U, psi, dims, bc), 64)
     refM = H.half_of(oracle.apply_M(U, psi, dims, bc, c["kappa"], 1), dims, 0)
-    assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), c["kappa"], 1), refM) <= TOL[64]
+    H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), c["kappa"], 1), refM, 64)
 
 
 def test_config2_gamma5_hermiticity_and_covariance(H):
@@ -92,7 +92,7 @@ def test_config2_gamma5_hermiticity_and_covariance(H):
     g2 = H.Gpu(dims, 64, 12, bc, Ug)
     psig = np.einsum("...ab,...sb->...sa", gx, psi)
     expect = np.einsum("...ab,...sb->...sa", gx, g.dslash_full(psi))
-    assert H.rel_l2(g2.dslash_full(psig), expect) <= 1e-12
+    H.assert_parity(g2.dslash_full(psig), expect, 64)
 
 
 # ------------------------------------------------------------------ config 3: 16^3x32 full, fp32 + fp64
@@ -101,9 +101,9 @@ def test_config3_full(H, precision, recon):
     c, U, psi = _inputs(3, precision)
     dims, bc = c["dims"], c["bc"]
     g = H.Gpu(dims, precision, recon, bc, U)
-    assert H.rel_l2(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc)) <= TOL[precision]
+    H.assert_parity(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc), precision)
     refM = oracle.apply_M(U, psi, dims, bc, c["kappa"], 0)
-    assert H.rel_l2(g.apply_M(psi, c["kappa"], 0), refM) <= TOL[precision]
+    H.assert_parity(g.apply_M(psi, c["kappa"], 0), refM, precision)
 
 
 # ------------------------------------------------------------------ edge cases
@@ -117,14 +117,12 @@ def test_ragged_anisotropic_complex_bc(H, precision, recon):
     U = li.random_su3_links(dims, seed=21).astype(cdtype(precision))
     psi = li.gaussian_spinor(dims, seed=22).astype(cdtype(precision))
     g = H.Gpu(dims, precision, recon, bc, U)
-    for blk in (64, 128):
-        g.ctx.set_block_threads(blk)
-        assert H.rel_l2(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc)) <= TOL[precision]
-        for op in (0, 1):
-            ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, op), dims, op)
-            assert H.rel_l2(g.dslash_eo(H.half_of(psi, dims, 1 - op), op), ref) <= TOL[precision]
+    H.assert_parity(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc), precision)
+    for op in (0, 1):
+        ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, op), dims, op)
+        H.assert_parity(g.dslash_eo(H.half_of(psi, dims, 1 - op), op), ref, precision)
     refM = H.half_of(oracle.apply_M(U, psi, dims, bc, 0.13, 1), dims, 0)
-    assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), 0.13, 1), refM) <= TOL[precision]
+    H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), 0.13, 1), refM, precision)
 
 
 @pytest.mark.parametrize("dims", [(6, 6, 6, 6), (4, 6, 6, 6), (6, 4, 6, 10)])
@@ -138,12 +136,12 @@ def test_ragged_last_tile(H, dims, precision, recon):
     bc = (1, 1, 1, -1)
     g = H.Gpu(dims, precision, recon, bc, U)
     assert np.prod(dims) // 2 % 32 != 0
-    assert H.rel_l2(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc)) <= TOL[precision]
+    H.assert_parity(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc), precision)
     for op in (0, 1):
         ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, op), dims, op)
-        assert H.rel_l2(g.dslash_eo(H.half_of(psi, dims, 1 - op), op), ref) <= TOL[precision]
+        H.assert_parity(g.dslash_eo(H.half_of(psi, dims, 1 - op), op), ref, precision)
     refM = H.half_of(oracle.apply_M(U, psi, dims, bc, 0.14, 1), dims, 0)
-    assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), 0.14, 1), refM) <= TOL[precision]
+    H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), 0.14, 1), refM, precision)
     # pack -> unpack round trip is bit exact on the ragged layout too
     assert np.array_equal(g.from_native(g.to_native(psi, -1), -1), psi)
 
@@ -154,7 +152,7 @@ def test_minimum_extent_and_all_periodic(H):
     psi = li.gaussian_spinor(dims, seed=32)
     for bc in [(1, 1, 1, 1), (-1, -1, -1, -1)]:
         g = H.Gpu(dims, 64, 12, bc, U)
-        assert H.rel_l2(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc)) <= TOL[64]
+        H.assert_parity(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc), 64)
 
 
 def test_pack_unpack_roundtrip_bit_exact(H):
@@ -182,9 +180,27 @@ def test_error_codes(H):
     with pytest.raises(L.LqcdError) as e:
         g.ctx.dslash_eo(a, g.gauge, b, 2)
     assert e.value.status == L.LQCD_EINVAL
-    with pytest.raises(L.LqcdError) as e:
-        g.ctx.dslash_eo(a.data_ptr() + 8, g.gauge, b, 0)
-    assert e.value.status == L.LQCD_EALIGN
+    # native fields are read and written with 256-bit words: anything short of 32-byte alignment is refused with a
+    # return code (never a misaligned-address fault); the context stays usable afterwards
+    ws, full, full2 = g.buf(), g.buf(half=False), g.buf(half=False)
+    c = torch.empty((g.ctx.Vh, 4, 3), dtype=torch.complex128, device="cuda:0")
+    for off in (8, 16, 24):
+        for call in (lambda: g.ctx.dslash_eo(a.data_ptr() + off, g.gauge, b, 0),
+                     lambda: g.ctx.dslash_eo(a, g.gauge, b.data_ptr() + off, 0),
+                     lambda: g.ctx.dslash_eo(a, g.gauge.data_ptr() + off, b, 0),
+                     lambda: g.ctx.dslash_full(full.data_ptr() + off, g.gauge, full2),
+                     lambda: g.ctx.dslash_full(full, g.gauge, full2.data_ptr() + off),
+                     lambda: g.ctx.apply_M(a.data_ptr() + off, g.gauge, b, 0.1, 1, ws),
+                     lambda: g.ctx.apply_M(a, g.gauge, b, 0.1, 1, ws.data_ptr() + off),
+                     lambda: g.ctx.apply_M(full, g.gauge.data_ptr() + off, full2, 0.1, 0, None),
+                     lambda: g.ctx.pack_spinor(a.data_ptr() + off, c, 0),
+                     lambda: g.ctx.unpack_spinor(c, a.data_ptr() + off, 0)):
+            with pytest.raises(L.LqcdError) as e:
+                call()
+            assert e.value.status == L.LQCD_EALIGN
+    torch.cuda.synchronize()
+    g.ctx.dslash_eo(a, g.gauge, b, 0)   # no sticky error was raised
+    torch.cuda.synchronize()
     with pytest.raises(L.LqcdError) as e:
         g.ctx.apply_M(a, g.gauge, b, 0.1, 1, None)
     assert e.value.status == L.LQCD_EINVAL
@@ -208,9 +224,9 @@ def test_twisted_mass_matrix(H, precision, recon):
         g = H.Gpu(dims, precision, recon, bc, U)
         for mu in (0.25, -0.4):
             ref = oracle.apply_M_tm(U, psi, dims, bc, kappa, mu, 0)
-            assert H.rel_l2(g.apply_M(psi, kappa, 0, mu=mu), ref) <= TOL[precision]
+            H.assert_parity(g.apply_M(psi, kappa, 0, mu=mu), ref, precision)
             ref = H.half_of(oracle.apply_M_tm(U, psi, dims, bc, kappa, mu, 1), dims, 0)
-            assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), kappa, 1, mu=mu), ref) <= TOL[precision]
+            H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), kappa, 1, mu=mu), ref, precision)
         # mu = 0 is lqcd_apply_M bit for bit
         a = g.apply_M(H.half_of(psi, dims, 0), kappa, 1, mu=0.0)
         b = g.apply_M(H.half_of(psi, dims, 0), kappa, 1)
@@ -348,11 +364,11 @@ def test_fp32_spinors_with_half_links(H):
     Uq = _quantise_links(U)
     for op in (0, 1):
         got = g.dslash_eo(H.half_of(psi, dims, 1 - op), op)
-        assert H.rel_l2(got, H.half_of(oracle.dslash_eo(Uq, psi, dims, bc, op), dims, op)) <= TOL[32]
+        H.assert_parity(got, H.half_of(oracle.dslash_eo(Uq, psi, dims, bc, op), dims, op), 32)
         err = H.rel_l2(got, H.half_of(oracle.dslash_eo(U, psi, dims, bc, op), dims, op))
         assert 1e-5 < err <= 1e-3
     refT = H.half_of(oracle.apply_M_tm(Uq, psi, dims, bc, 0.15, 0.3, 1), dims, 0)
-    assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), 0.15, 1, mu=0.3), refT) <= TOL[32]
+    H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), 0.15, 1, mu=0.3), refT, 32)
     import paper_1112_5280_b200 as L
     with pytest.raises(L.LqcdError) as e:
         L.Context(dims, 64, 12, bc, 16)

@@ -55,7 +55,7 @@ def test_time_slabs_reproduce_the_whole_lattice(world, precision, recon, bc):
             got[s.t0:s.t0 + s.Tl] = local[1:s.Tl + 1]
         assert np.isfinite(got.view(np.float64 if precision == 64 else np.float32)).all()
         assert np.array_equal(got, ref_gpu), (world, gp)
-        assert H.rel_l2(got, oracle.dslash_eo(U, psi, dims, bc, gp)) <= (1e-12 if precision == 64 else 1e-5)
+        H.assert_parity(H.half_of(got, dims, gp), H.half_of(oracle.dslash_eo(U, psi, dims, bc, gp), dims, gp), precision)
 
 
 def test_slab_argument_checks():
