@@ -47,7 +47,9 @@
  *     links        gathered by output site: [parity p of x][tile][hop k 8][word][32][lane], hop k = 2 mu holds
  *                  U_mu(x), k = 2 mu + 1 holds U_mu(x - mu^) (stored as is; the kernel takes the adjoint).
  *                  Words of 4 floats (precision 32 recon 12, 3 words), 2 floats (precision 32 recon 18, 9 words),
- *                  4 doubles (precision 64 recon 12, 3 words) or 2 doubles (precision 64 recon 18, 9 words).  Every link is stored twice (capacity for contiguity: all
+ *                  4 doubles (precision 64 recon 12, 3 words) or 2 doubles (precision 64 recon 18, 9 words); recon 8: 2
+                  words of 4 reals (Re U01, Im U01, Re U02, Im U02 | Re U10, Im U10, arg U00 / pi, arg U20 / pi).
+                  Every link is stored twice (capacity for contiguity: all
  *                  8 links of a warp's 32 sites form one contiguous block); one application of
  *                  lqcd_dslash_eo still reads 8 links per output site exactly once.
  */
@@ -76,8 +78,12 @@ typedef struct {
     int precision;    /* 64 or 32: storage and arithmetic type of all fields; 16: fields stored as IEEE half
                          (spinors normalised per site, with an fp32 norm), fp32 arithmetic, recon 12 only;
                          canonical buffers are complex64; the CG entry points return LQCD_EUNSUPPORTED */
-    int recon;        /* 18 or 12: stored reals per link; 12 = two rows, third rebuilt in
-                         registers as conj(row0 x row1) ("RECONSTRUCT TWELVE") */
+    int recon;        /* 18, 12 or 8: stored reals per link; 12 = two rows, third rebuilt in
+                         registers as conj(row0 x row1) ("RECONSTRUCT TWELVE"); 8 = the minimal
+                         parametrisation of ref. [3]: U01, U02, U10 and the phases of U00, U20,
+                         the rest rebuilt in registers from unitarity and det = 1 (precision 32 / 64 only).
+                         Singular where |U00| = 1: unit links cannot be stored with recon 8, and a link loses
+                         digits like eps / min(|U00|, sqrt(1 - |U00|^2), |U20|) -- see lqcd_gauge_recon8_margin */
     double bc_re[4];  /* boundary phase bc_mu = bc_re + i bc_im, |bc_mu| = 1 within 1e-12; */
     double bc_im[4];  /* periodic (1,0), antiperiodic (-1,0), any U(1) phase allowed        */
     int link_precision; /* 0: links stored like the spinors.  16 with precision 32 and recon 12: fp32 spinors,
@@ -108,6 +114,13 @@ lqcd_status lqcd_pack_spinor(const lqcd_ctx* ctx, void* native_dev, const void* 
                              void* stream);
 lqcd_status lqcd_unpack_spinor(const lqcd_ctx* ctx, void* canonical_dev, const void* native_dev, int parity,
                                void* stream);
+
+/* min over all links of min(|U00|, sqrt(|U01|^2 + |U02|^2), |U20|) for a canonical link field on the device: the
+ * moduli the 8-real decoder obtains from differences and divides by.  0 means the field cannot be stored with
+ * recon 8 (e.g. unit links); otherwise the worst link is accurate to about eps / margin.  scratch_dev: 8 bytes of
+ * device memory, 8-byte aligned.  Synchronises `stream`; *margin_host is host memory. */
+lqcd_status lqcd_gauge_recon8_margin(const lqcd_ctx* ctx, const void* canonical_dev, void* scratch_dev,
+                                     double* margin_host, void* stream);
 
 /* ---- hot path: device pointers, native layout ---- */
 

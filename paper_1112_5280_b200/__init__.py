@@ -14,12 +14,13 @@ from . import _build
 
 LQCD_OK, LQCD_EINVAL, LQCD_EALIGN, LQCD_EALIAS, LQCD_EUNSUPPORTED, LQCD_ECUDA = range(6)
 PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, -1
+HAS_RECON8 = True
 
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
     "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_set_time_slab", "lqcd_dslash_eo_range", "lqcd_time_slice_bytes", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_dslash_eo_host_batch", "lqcd_launch_count",
-    "lqcd_status_string", "lqcd_last_cuda_error",
+    "lqcd_gauge_recon8_margin", "lqcd_status_string", "lqcd_last_cuda_error",
 ]
 
 
@@ -75,6 +76,7 @@ def _lib():
         lib.lqcd_cg_solve_tm.argtypes = [vp, vp, vp, vp, cd, cd, cd, ci, vp, ctypes.POINTER(ci), ctypes.POINTER(cd), vp]
         lib.lqcd_dslash_eo_host.argtypes = [vp, vp, vp, vp, ci, vp, vp]
         lib.lqcd_dslash_eo_host_batch.argtypes = [vp, ci, ctypes.POINTER(vp), vp, ctypes.POINTER(vp), ctypes.POINTER(ci), vp, vp]
+        lib.lqcd_gauge_recon8_margin.argtypes = [vp, vp, vp, ctypes.POINTER(cd), vp]
         lib.lqcd_launch_count.argtypes = []
         lib.lqcd_launch_count.restype = ctypes.c_ulonglong
         lib.lqcd_status_string.argtypes = [ci]
@@ -138,6 +140,12 @@ class Context:
     # layout conversion
     def pack_gauge(self, native, canonical, stream=None):
         _chk(_lib().lqcd_pack_gauge(self._h, _ptr(native), _ptr(canonical), _stream(stream)), "lqcd_pack_gauge")
+
+    def gauge_recon8_margin(self, canonical, scratch, stream=None):
+        m = ctypes.c_double(0.0)
+        _chk(_lib().lqcd_gauge_recon8_margin(self._h, _ptr(canonical), _ptr(scratch), ctypes.byref(m), _stream(stream)),
+             "lqcd_gauge_recon8_margin")
+        return m.value
 
     def pack_spinor(self, native, canonical, parity, stream=None):
         _chk(_lib().lqcd_pack_spinor(self._h, _ptr(native), _ptr(canonical), int(parity), _stream(stream)),

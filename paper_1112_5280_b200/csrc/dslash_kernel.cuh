@@ -50,16 +50,11 @@ template <> struct Proj<3> { static constexpr int ja = 2, ca = C_P1, jb = 3, cb 
 
 template <typename R> struct BcPhases { R re[4], im[4]; };
 
-// The arithmetic of one of the eight hops on a gathered neighbour spinor v and link u:
-// project (K3), boundary phase (K3b), colour multiply (K4), reconstruct + accumulate (K5).
-template <typename R, bool CBC, int MU, bool FWD>
-__device__ __forceinline__ void hop_math(R acc[24], const R v[24], R scale, const R u[18], bool cross,
-                                         const BcPhases<R>& bc) {
-    constexpr int S = FWD ? +1 : -1;
+// K3: half spinor h[spin 2][colour 3][reim] = the upper two components of (1 -+ gamma_mu) psi for the forward /
+// backward hop (S = +1 / -1), from a gathered neighbour spinor v.
+template <typename R, int MU, int S>
+__device__ __forceinline__ void project(const R v[24], R h[12]) {
     using P = Proj<MU>;
-
-    // K3: half spinor h[spin 2][colour 3][reim]
-    R h[12];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         R r0 = v[2 * c], i0 = v[2 * c + 1];
@@ -69,6 +64,44 @@ __device__ __forceinline__ void hop_math(R acc[24], const R v[24], R scale, cons
         h[2 * c] = r0; h[2 * c + 1] = i0;
         h[6 + 2 * c] = r1; h[6 + 2 * c + 1] = i1;
     }
+}
+
+// K3 on 16-bit storage with Blackwell's mixed-precision adds (add/sub.rn.f32.f16 -> FHADD: an f16 operand taken from
+// either half of a register plus an f32 operand, exact fp32 result): the lower spin component is converted (12
+// conversions per hop instead of 24) and the upper one enters the add as f16, so the projection costs no rounding and
+// no instruction beyond the conversion it replaces.  w: the 3 16-byte words of the site, complex k = 3 spin + colour
+// in 32-bit register k (low half re, high half im).
+__device__ __forceinline__ float fhadd(unsigned short a, float c) { float r; asm("add.rn.f32.f16 %0, %1, %2;" : "=f"(r) : "h"(a), "f"(c)); return r; }
+__device__ __forceinline__ float fhsub(unsigned short a, float c) { float r; asm("sub.rn.f32.f16 %0, %1, %2;" : "=f"(r) : "h"(a), "f"(c)); return r; }
+
+// (re, im) = a + C b for a unit coefficient C; a, b packed half2 (re low, im high)
+template <int C>
+__device__ __forceinline__ void cmix_h(unsigned a, unsigned b, float& re, float& im) {
+    const unsigned short ar = (unsigned short)(a & 0xffffu), ai = (unsigned short)(a >> 16);
+    const float2 bf = __half22float2(*reinterpret_cast<const __half2*>(&b));
+    if (C == C_P1) { re = fhadd(ar, bf.x); im = fhadd(ai, bf.y); }
+    else if (C == C_M1) { re = fhsub(ar, bf.x); im = fhsub(ai, bf.y); }
+    else if (C == C_PI) { re = fhsub(ar, bf.y); im = fhadd(ai, bf.x); }
+    else { re = fhadd(ar, bf.y); im = fhsub(ai, bf.x); }
+}
+
+template <int MU, int S>
+__device__ __forceinline__ void project_h(const uint4 w[3], float h[12]) {
+    using P = Proj<MU>;
+    const unsigned* k = reinterpret_cast<const unsigned*>(w);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        cmix_h<coef_sgn<S>(P::ca)>(k[c], k[3 * P::ja + c], h[2 * c], h[2 * c + 1]);
+        cmix_h<coef_sgn<S>(P::cb)>(k[3 + c], k[3 * P::jb + c], h[6 + 2 * c], h[6 + 2 * c + 1]);
+    }
+}
+
+// The rest of the arithmetic of one hop on the projected half spinor h and the link u:
+// boundary phase (K3b), colour multiply (K4), reconstruct + accumulate (K5).
+template <typename R, bool CBC, int MU, bool FWD>
+__device__ __forceinline__ void hop_rest(R acc[24], R h[12], R scale, const R u[18], bool cross, const BcPhases<R>& bc) {
+    constexpr int S = FWD ? +1 : -1;
+    using P = Proj<MU>;
 
     // K3b: psi(x + L mu^) = bc psi(x): forward crossing multiplies by bc_mu, backward by conj(bc_mu).
     // Real (+-1) phases cost nothing: the sign f rides on the accumulation FMAs of K5.
@@ -128,6 +161,11 @@ __device__ __forceinline__ void hop_math(R acc[24], const R v[24], R scale, cons
     }
 }
 
+// 16-bit storage: project with mixed-precision adds on the stored words (1) or convert all 24 components first (0)
+#ifndef LQCD_F16_MIXED
+#define LQCD_F16_MIXED 1
+#endif
+
 // Hop K = 2 mu + (backward ? 1 : 0): gather the neighbour spinor and the link stored for this hop
 // (U_mu(x) or U_mu(x - mu^), fields.cuh), then the arithmetic.  S = storage type, R = arithmetic type.
 template <typename S, int RECON, bool CBC, int K>
@@ -138,10 +176,65 @@ __device__ __forceinline__ void hop_step(typename Compute<S>::type acc[24],
     using R = typename Compute<S>::type;
     constexpr int MU = K / 2;
     constexpr bool FWD = (K & 1) == 0;
-    R v[24], u[18], scale;
-    load_field<S>(in, ntiles, nb[K], v, scale);
+    R h[12], u[18], scale;
+    if constexpr (sizeof(S) == 2 && LQCD_F16_MIXED) {
+        uint4 w[3];
+        load_words_h(in, ntiles, nb[K], w, scale);
+        project_h<MU, FWD ? +1 : -1>(w, h);
+    } else {
+        R v[24];
+        load_field<S>(in, ntiles, nb[K], v, scale);
+        project<R, MU, FWD ? +1 : -1>(v, h);
+    }
     if constexpr (half_links<S, RECON>) load_link_h(site_links, K, u); else load_link<R, RECON>(site_links, K, u);
-    hop_math<R, CBC, MU, FWD>(acc, v, scale, u, (crossmask >> K) & 1u, bc);
+    hop_rest<R, CBC, MU, FWD>(acc, h, scale, u, (crossmask >> K) & 1u, bc);
+}
+
+// Experiment (north_star (3) "warp shuffles where they pay"): the two x hops without a second
+// gather.  In the opposite-parity array the +-x neighbours of site cb are cb itself and cb + 1 (x odd) or cb - 1
+// (x even): every lane loads its "centre" spinor in[cb] once, projects it both ways (A = (1 - gamma_x) psi, what a
+// forward hop needs; B = (1 + gamma_x) psi, what a backward hop needs), keeps the one its own hop needs and hands the
+// other to the lane that needs it with 12 (fp32) / 24 (fp64) register shuffles.  A lane whose neighbour lives in
+// another warp tile gathers it from memory as before.  Off by default: measured slower.
+#ifndef LQCD_SHFL_X
+#define LQCD_SHFL_X 0
+#endif
+
+template <typename R>
+__device__ __forceinline__ R shfl_(R v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+
+template <typename R, int RECON, bool CBC>
+__device__ __forceinline__ void hops_x_shuffled(R acc[24], const typename LinkStore<R, RECON>::word* __restrict__ site_links,
+                                                const R* __restrict__ in, int cb, int cb_end, int x_odd, const int nb[8],
+                                                unsigned crossmask, const BcPhases<R>& bc) {
+    R vc[24], A[12], B[12];
+    load_spinor<R>(in, cb, vc);
+    project<R, 0, +1>(vc, A);
+    project<R, 0, -1>(vc, B);
+    // the neighbour that is not the centre: forward (x odd) or backward (x even); its lane if it is in this warp's tile
+    const int other = x_odd ? nb[0] : nb[1];
+    const int src = other - (cb - (int)(threadIdx.x & 31u));   // lane l of the warp works on site (warp base + l)
+    const bool in_warp = src >= 0 && src < 32 && other < cb_end;  // ... if that site is inside this launch's range
+    R recv[12];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) recv[k] = shfl_<R>(x_odd ? A[k] : B[k], in_warp ? src : 0);
+    // lanes handing to a lane of the other row kind would send the wrong projection: x_odd is constant along an x row
+    // and the neighbour is always in the same row, so sender and receiver agree.
+    if (!in_warp) {
+        R vo[24];
+        load_spinor<R>(in, other, vo);
+        if (x_odd) project<R, 0, +1>(vo, recv); else project<R, 0, -1>(vo, recv);
+    }
+    R hf[12], hb[12], u[18];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+        hf[k] = x_odd ? recv[k] : A[k];
+        hb[k] = x_odd ? B[k] : recv[k];
+    }
+    load_link<R, RECON>(site_links, 0, u);
+    hop_rest<R, CBC, 0, true>(acc, hf, (R)1, u, (crossmask >> 0) & 1u, bc);
+    load_link<R, RECON>(site_links, 1, u);
+    hop_rest<R, CBC, 0, false>(acc, hb, (R)1, u, (crossmask >> 1) & 1u, bc);
 }
 
 // Resident 64-thread blocks per SM promised to ptxas (__launch_bounds__ min blocks).  The hint sets the
@@ -163,12 +256,20 @@ __device__ __forceinline__ void hop_step(typename Compute<S>::type acc[24],
 #ifndef LQCD_MINB_F16_R12
 #define LQCD_MINB_F16_R12 8
 #endif
+#ifndef LQCD_MINB_F32_R8
+#define LQCD_MINB_F32_R8 8
+#endif
+#ifndef LQCD_MINB_F64_R8
+#define LQCD_MINB_F64_R8 6
+#endif
 template <typename R, int RECON> struct MinBlocks;
 template <> struct MinBlocks<float, 12>  { static constexpr int value = LQCD_MINB_F32_R12; };
 template <> struct MinBlocks<float, 18>  { static constexpr int value = LQCD_MINB_F32_R18; };
 template <> struct MinBlocks<double, 12> { static constexpr int value = LQCD_MINB_F64_R12; };
 template <> struct MinBlocks<double, 18> { static constexpr int value = LQCD_MINB_F64_R18; };
 template <> struct MinBlocks<__half, 12>  { static constexpr int value = LQCD_MINB_F16_R12; };
+template <> struct MinBlocks<float, 8>   { static constexpr int value = LQCD_MINB_F32_R8; };
+template <> struct MinBlocks<double, 8>  { static constexpr int value = LQCD_MINB_F64_R8; };
 #ifndef LQCD_MINB_F32_R12H
 #define LQCD_MINB_F32_R12H 8
 #endif
@@ -215,8 +316,14 @@ dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restr
         out += (size_t)p * half;
         if (XPAY) xin += (size_t)p * half;
     }
-    const int cb = cb_begin + blockIdx.x * BLOCK + threadIdx.x;  // [cb_begin, cb_end): all sites, or a range of time slices
-    if (cb >= cb_end) return;
+    int cb = cb_begin + blockIdx.x * BLOCK + threadIdx.x;  // [cb_begin, cb_end): all sites, or a range of time slices
+    constexpr bool SHFLX = LQCD_SHFL_X && sizeof(S) != 2 && !half_links<S, RECON>;
+    bool live = true;
+    if (cb >= cb_end) {
+        if constexpr (!SHFLX) return;
+        live = false;     // with shuffles every lane of the warp stays: a dead lane works on the last site and stores nothing
+        cb = cb_end - 1;
+    }
     const Site s = decode_site(g, cb, p);
 
     // K1: all eight neighbours and boundary-crossing flags
@@ -240,8 +347,12 @@ dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restr
 #pragma unroll
     for (int k = 0; k < 24; ++k) acc[k] = 0;
 
-    hop_step<S, RECON, CBC, 0>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
-    hop_step<S, RECON, CBC, 1>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
+    if constexpr (SHFLX) {
+        hops_x_shuffled<R, RECON, CBC>(acc, site_links, in, cb, cb_end, s.x_odd, nb, crossmask, bc);
+    } else {
+        hop_step<S, RECON, CBC, 0>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
+        hop_step<S, RECON, CBC, 1>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
+    }
     hop_step<S, RECON, CBC, 2>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
     hop_step<S, RECON, CBC, 3>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
     hop_step<S, RECON, CBC, 4>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
@@ -265,7 +376,7 @@ dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restr
 #pragma unroll
         for (int k = 12; k < 24; ++k) acc[k] = -acc[k];
     }
-    store_field<S>(out, g.ntiles, cb, acc);
+    if (live) store_field<S>(out, g.ntiles, cb, acc);
 }
 
 }  // namespace lqcd

@@ -40,6 +40,8 @@ template <> struct LinkWord<float, 18>  { using type = float2;   static constexp
 template <> struct LinkWord<double, 12> { using type = double4_; static constexpr int LW = 4; };
 template <> struct LinkWord<double, 18> { using type = double2;  static constexpr int LW = 2; };
 template <> struct LinkWord<float, 13>  { using type = float4;   static constexpr int LW = 4; };  // RECON_12H: unused (half links)
+template <> struct LinkWord<float, 8>   { using type = float4;   static constexpr int LW = 4; };  // 8-real: 2 x 16 B
+template <> struct LinkWord<double, 8>  { using type = double4_; static constexpr int LW = 4; };  // 8-real: 2 x 32 B
 
 __device__ __forceinline__ void unpack(const float4& w, float* v)  { v[0] = w.x; v[1] = w.y; v[2] = w.z; v[3] = w.w; }
 __device__ __forceinline__ void unpack(const float2& w, float* v)  { v[0] = w.x; v[1] = w.y; }
@@ -160,6 +162,40 @@ __device__ __forceinline__ void recon_row2(R u[18]) {
     }
 }
 
+// 8-real storage (next row f4, ref. [3] at :139): with the rows of U called a, b, c the stored reals are
+//   r = (Re a1, Im a1, Re a2, Im a2, Re b0, Im b0, arg(a0) / pi, arg(c0) / pi)
+// and, with N2 = |a1|^2 + |a2|^2:  a0 = sqrt(1 - N2) e^{i pi r6},  c0 = sqrt(N2 - |b0|^2) e^{i pi r7},
+//   b1 = -(a1 conj(a0) b0 + conj(a2 c0)) / N2,   b2 = (conj(a1 c0) - a2 conj(a0) b0) / N2,   c = conj(a x b).
+// (rows orthonormal, det = 1; the 2 x 2 system for b1, b2 has determinant N2.)  Singular for N2 = 0, i.e. |U00| = 1:
+// unit links cannot be stored this way (lqcd_gauge_recon8_margin reports how close a field comes).
+__device__ __forceinline__ void sincospi_(float x, float& s, float& c) { sincospif(x, &s, &c); }
+__device__ __forceinline__ void sincospi_(double x, double& s, double& c) { sincospi(x, &s, &c); }
+__device__ __forceinline__ float sqrt_(float x) { return sqrtf(x); }
+__device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
+
+template <typename R>
+__device__ __forceinline__ void recon8(const R r[8], R u[18]) {
+    const R a1r = r[0], a1i = r[1], a2r = r[2], a2i = r[3], b0r = r[4], b0i = r[5];
+    const R N2 = fmar(a1r, a1r, fmar(a1i, a1i, fmar(a2r, a2r, a2i * a2i)));
+    const R B2 = fmar(b0r, b0r, b0i * b0i);
+    R s0, c0, s2, c2;
+    sincospi_(r[6], s0, c0);
+    sincospi_(r[7], s2, c2);
+    const R ma = sqrt_(fmax((R)1 - N2, (R)0)), mc = sqrt_(fmax(N2 - B2, (R)0));
+    const R a0r = ma * c0, a0i = ma * s0, c0r = mc * c2, c0i = mc * s2;
+    const R inv = (R)1 / N2;
+    // t = conj(a0) b0;  w = a2 c0;  v = a1 c0
+    const R tr = fmar(a0r, b0r, a0i * b0i), ti = fmar(a0r, b0i, -a0i * b0r);
+    const R wr = fmar(a2r, c0r, -a2i * c0i), wi = fmar(a2r, c0i, a2i * c0r);
+    const R vr = fmar(a1r, c0r, -a1i * c0i), vi = fmar(a1r, c0i, a1i * c0r);
+    // b1 = -(a1 t + conj(w)) / N2;  b2 = (conj(v) - a2 t) / N2
+    const R b1r = -inv * (fmar(a1r, tr, -a1i * ti) + wr), b1i = -inv * (fmar(a1r, ti, a1i * tr) - wi);
+    const R b2r = inv * (vr - fmar(a2r, tr, -a2i * ti)), b2i = inv * (-vi - fmar(a2r, ti, a2i * tr));
+    u[0] = a0r; u[1] = a0i; u[2] = a1r; u[3] = a1i; u[4] = a2r; u[5] = a2i;
+    u[6] = b0r; u[7] = b0i; u[8] = b1r; u[9] = b1i; u[10] = b2r; u[11] = b2i;
+    recon_row2<R>(u);
+}
+
 // ---- 16-bit storage (next row f4; "RECONSTRUCT TWELVE [3]" and the half-precision storage of ref. [3],
 // PAPER.md:89, :139): fields are stored as IEEE half, the arithmetic stays fp32 --------------------------------
 //   half spinor: 24 halfs = 3 16-byte words per site, [tile][q 3][32] as above, holding v / n(x) with
@@ -193,6 +229,15 @@ __device__ __forceinline__ void load_spinor_h(const __half* __restrict__ base, i
         const uint4 w = __ldg(p + q * TILE);
         unpack_h8(w, v + 8 * q);
     }
+}
+
+// the stored words themselves (for the mixed-precision projection of dslash_kernel.cuh) and the site norm
+__device__ __forceinline__ void load_words_h(const __half* __restrict__ base, int ntiles, int cb, uint4 w[3], float& n) {
+    const uint4* words = reinterpret_cast<const uint4*>(base);
+    const uint4* p = words + (size_t)(cb / TILE) * (HALF_Q * TILE) + (cb % TILE);
+    n = __ldg(reinterpret_cast<const float*>(words + half_spinor_words(ntiles)) + cb);
+#pragma unroll
+    for (int q = 0; q < HALF_Q; ++q) w[q] = __ldg(p + q * TILE);
 }
 
 __device__ __forceinline__ void store_spinor_h(__half* __restrict__ base, int ntiles, int cb, const float v[24]) {
@@ -280,12 +325,22 @@ template <typename R, int RECON>
 __device__ __forceinline__ void load_link(const typename LinkWord<R, RECON>::type* __restrict__ site_links, int k, R u[18]) {
     using LWd = typename LinkWord<R, RECON>::type;
     constexpr int LW = LinkWord<R, RECON>::LW, NW = RECON / LW;
+    if constexpr (RECON == 8) {
+        R r[8];
 #pragma unroll
-    for (int w = 0; w < NW; ++w) {
-        LWd x = ld_stream(site_links + (k * NW + w) * TILE);
-        unpack(x, u + w * LW);
+        for (int w = 0; w < NW; ++w) {
+            LWd x = ld_stream(site_links + (k * NW + w) * TILE);
+            unpack(x, r + w * LW);
+        }
+        recon8<R>(r, u);
+    } else {
+#pragma unroll
+        for (int w = 0; w < NW; ++w) {
+            LWd x = ld_stream(site_links + (k * NW + w) * TILE);
+            unpack(x, u + w * LW);
+        }
+        if constexpr (RECON == 12) recon_row2<R>(u);
     }
-    if constexpr (RECON == 12) recon_row2<R>(u);
 }
 
 }  // namespace lqcd

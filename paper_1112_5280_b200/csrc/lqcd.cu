@@ -22,6 +22,8 @@ extern template lqcd_status launch_recon<float, 12>(LQCD_LAUNCH_RECON_ARGS);
 extern template lqcd_status launch_recon<float, 18>(LQCD_LAUNCH_RECON_ARGS);
 extern template lqcd_status launch_recon<__half, 12>(LQCD_LAUNCH_RECON_ARGS);
 extern template lqcd_status launch_recon<float, RECON_12H>(LQCD_LAUNCH_RECON_ARGS);
+extern template lqcd_status launch_recon<double, 8>(LQCD_LAUNCH_RECON_ARGS);
+extern template lqcd_status launch_recon<float, 8>(LQCD_LAUNCH_RECON_ARGS);
 }  // namespace lqcd
 
 namespace {
@@ -71,9 +73,11 @@ lqcd_status launch_dslash(const lqcd_ctx* c, void* out, const void* gauge, const
     if (c->p.precision == 16) return launch_recon<__half, 12>(c, out, gauge, in, xin, e, parity, st, rg);
     if (c->p.precision == 32) {
         if (c->p.link_precision == 16) return launch_recon<float, RECON_12H>(c, out, gauge, in, xin, e, parity, st, rg);
+        if (c->p.recon == 8) return launch_recon<float, 8>(c, out, gauge, in, xin, e, parity, st, rg);
         return c->p.recon == 12 ? launch_recon<float, 12>(c, out, gauge, in, xin, e, parity, st, rg)
                                 : launch_recon<float, 18>(c, out, gauge, in, xin, e, parity, st, rg);
     }
+    if (c->p.recon == 8) return launch_recon<double, 8>(c, out, gauge, in, xin, e, parity, st, rg);
     return c->p.recon == 12 ? launch_recon<double, 12>(c, out, gauge, in, xin, e, parity, st, rg)
                             : launch_recon<double, 18>(c, out, gauge, in, xin, e, parity, st, rg);
 }
@@ -92,10 +96,11 @@ extern "C" {
 lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p) {
     if (!ctx || !p) return LQCD_EINVAL;
     if (p->precision != 16 && p->precision != 32 && p->precision != 64) return LQCD_EINVAL;
-    if (p->recon != 12 && p->recon != 18) return LQCD_EINVAL;
+    if (p->recon != 8 && p->recon != 12 && p->recon != 18) return LQCD_EINVAL;
     if (p->precision == 16 && p->recon != 12) return LQCD_EUNSUPPORTED;  // 16-bit storage: 12-real links only
     if (p->link_precision != 0 && p->link_precision != 16 && p->link_precision != p->precision) return LQCD_EINVAL;
     if (p->link_precision == 16 && (p->precision == 64 || p->recon != 12)) return LQCD_EUNSUPPORTED;
+    if (p->recon == 8 && p->precision == 16) return LQCD_EUNSUPPORTED;  // 8-real links: fp32 / fp64 storage only
     double vol = 1;
     bool cbc = false;
     for (int mu = 0; mu < 4; ++mu) {
@@ -151,6 +156,9 @@ lqcd_status lqcd_pack_gauge(const lqcd_ctx* c, void* native, const void* canon, 
     cudaStream_t st = (cudaStream_t)stream;
     if (c->p.precision == 16 || c->p.link_precision == 16) {
         pack_gauge_h_kernel<<<grid, 128, 0, st>>>((__half*)native, (const float*)canon, c->g);
+    } else if (c->p.recon == 8) {
+        if (c->p.precision == 32) pack_gauge8_kernel<float><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);
+        else pack_gauge8_kernel<double><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, c->g);
     } else if (c->p.precision == 32) {
         if (c->p.recon == 12) pack_gauge_kernel<float, 12><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);
         else pack_gauge_kernel<float, 18><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);
@@ -159,6 +167,27 @@ lqcd_status lqcd_pack_gauge(const lqcd_ctx* c, void* native, const void* canon, 
         else pack_gauge_kernel<double, 18><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, c->g);
     }
     return after_launch();
+}
+
+lqcd_status lqcd_gauge_recon8_margin(const lqcd_ctx* c, const void* canon, void* scratch, double* margin_host, void* stream) {
+    if (!c || !canon || !scratch || !margin_host) return LQCD_EINVAL;
+    if (c->p.precision == 16) return LQCD_EUNSUPPORTED;
+    if (!aligned16(canon) || (reinterpret_cast<uintptr_t>(scratch) & 7u)) return LQCD_EALIGN;
+    cudaStream_t st = (cudaStream_t)stream;
+    const double one = 1.0;
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(scratch, &one, sizeof(one), cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    const size_t nlinks = (size_t)8 * c->g.Vh;
+    const unsigned grid = (unsigned)((nlinks + 255) / 256);
+    if (c->p.precision == 64) recon8_margin_kernel<double><<<grid, 256, 0, st>>>((const double*)canon, nlinks, (unsigned long long*)scratch);
+    else recon8_margin_kernel<float><<<grid, 256, 0, st>>>((const float*)canon, nlinks, (unsigned long long*)scratch);
+    lqcd_status s = after_launch();
+    if (s != LQCD_OK) return s;
+    double m2 = 0.0;
+    if ((e = cudaMemcpyAsync(&m2, scratch, sizeof(m2), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+    *margin_host = std::sqrt(m2);
+    return LQCD_OK;
 }
 
 static lqcd_status pack_unpack(const lqcd_ctx* c, void* dst, const void* src, int parity, void* stream, bool unpack) {

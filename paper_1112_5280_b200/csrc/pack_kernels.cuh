@@ -41,6 +41,45 @@ __global__ void pack_gauge_kernel(R* __restrict__ native, const R* __restrict__ 
         for (int l = 0; l < LW; ++l) dst[(size_t)w * TILE * LW + l] = src[w * LW + l];
 }
 
+// 8-real storage (fields.cuh): r = (Re a1, Im a1, Re a2, Im a2, Re b0, Im b0, arg(a0) / pi, arg(c0) / pi), the two
+// phases evaluated in double and rounded once.  Same grid as pack_gauge_kernel.
+template <typename R>
+__global__ void pack_gauge8_kernel(R* __restrict__ native, const R* __restrict__ canon, Geom g) {
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= g.Vh) return;
+    const int k = blockIdx.y, p = blockIdx.z, mu = k >> 1;
+    const size_t V = (size_t)2 * g.Vh;
+    const size_t site = (k & 1) ? lex_back(g, cb, p, mu) : lex_of(g, cb, p);
+    const R* src = canon + ((size_t)mu * V + site) * 18;
+    constexpr double inv_pi = 0.31830988618379067154;
+    R r[8] = {src[2], src[3], src[4], src[5], src[6], src[7],
+              (R)(atan2((double)src[1], (double)src[0]) * inv_pi), (R)(atan2((double)src[13], (double)src[12]) * inv_pi)};
+    R* dst = native + link_word0<R, 8>(g.ntiles, p, cb, k) * 4;
+#pragma unroll
+    for (int w = 0; w < 2; ++w)
+#pragma unroll
+        for (int l = 0; l < 4; ++l) dst[(size_t)w * TILE * 4 + l] = r[w * 4 + l];
+}
+
+// min over all links of min(|a0|, sqrt(N2), |c0|)^2 -- the moduli the 8-real decoder derives from differences and
+// divides by; the result is the squared margin, kept as the bit pattern of a non-negative double (ordered like
+// unsigned integers) so that atomicMin applies.  grid: (ceil(4 V / block)).
+template <typename R>
+__global__ void recon8_margin_kernel(const R* __restrict__ canon, size_t nlinks, unsigned long long* __restrict__ out) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double m = 1.0;
+    if (i < nlinks) {
+        const R* u = canon + i * 18;
+        const double a0 = (double)u[0] * u[0] + (double)u[1] * u[1];
+        const double n2 = (double)u[2] * u[2] + (double)u[3] * u[3] + (double)u[4] * u[4] + (double)u[5] * u[5];
+        const double c0 = (double)u[12] * u[12] + (double)u[13] * u[13];
+        m = fmin(a0, fmin(n2, c0));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) atomicMin(out, (unsigned long long)__double_as_longlong(m));
+}
+
 // mode 0/1: canonical half spinor [Vh][4][3] of that parity <-> native half spinor.
 // mode -1 : canonical full spinor [V][4][3] <-> native full [even|odd]; blockIdx.y = parity.
 template <typename R, bool UNPACK>

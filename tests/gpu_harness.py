@@ -126,3 +126,20 @@ def assert_parity(a, ref, precision, l2_tol=None, site_tol=None, what=""):
     assert e2 <= l2_tol, f"{what}: rel-L2 {e2:.3e} > {l2_tol:g} (worst site {k}: {es:.3e})"
     assert es <= site_tol, f"{what}: per-site relative error {es:.3e} > {site_tol:g} at site {k} (rel-L2 {e2:.3e})"
     return e2, es
+
+
+def site_tol_for(U, precision, recon):
+    """Per-site bar of a run with `recon`-real links.  12 / 18: the common bar.  8: the worst link is decoded to about
+    8 eps / min(|U00|, sqrt(1 - |U00|^2), |U20|) (pins R3 / R5 of tests/test_oracle_recon8_pins.py), so the bar follows
+    the conditioning of the worst link of the field; never below the common bar."""
+    if recon != 8:
+        return SITE_TOL[precision]
+    m = np.minimum(np.minimum(np.abs(U[..., 0, 0]), np.sqrt(np.abs(U[..., 0, 1]) ** 2 + np.abs(U[..., 0, 2]) ** 2)),
+                   np.abs(U[..., 2, 0])).min()
+    eps = 2.0 ** -53 if precision == 64 else 2.0 ** -24
+    return max(SITE_TOL[precision], 16 * eps / float(m))
+
+
+def recon8_margin(U):
+    return float(np.minimum(np.minimum(np.abs(U[..., 0, 0]), np.sqrt(np.abs(U[..., 0, 1]) ** 2 + np.abs(U[..., 0, 2]) ** 2)),
+                            np.abs(U[..., 2, 0])).min())

@@ -41,12 +41,14 @@ def test_create_validation_and_sizes():
     c6 = L.Context((6, 6, 6, 6), 32, 12)  # Vh = 648 is padded to 21 tiles of 32 sites
     assert c6.spinor_bytes(True) == 21 * 32 * 24 * 4 and c6.gauge_bytes() == 2 * 21 * 32 * 8 * 12 * 4
     assert c.host_workspace_bytes() >= c.gauge_bytes() + 4 * 256 * 18 * 8 + 4 * c.spinor_bytes(True)
+    c8 = L.Context((8, 8, 8, 16), 64, 8)
+    assert c8.gauge_bytes() == 2 * 8 * 4096 * 8 * 8
     c16 = L.Context((8, 8, 8, 16), 16, 12)
     assert c16.spinor_bytes(True) == 4096 * 52 and c16.gauge_bytes() == 2 * 8 * 4096 * 24
     with pytest.raises(L.LqcdError) as e:
         L.Context((8, 8, 8, 16), 16, 18)
     assert e.value.status == L.LQCD_EUNSUPPORTED
-    for bad in [dict(dims=(4, 4, 3, 4)), dict(dims=(2, 4, 4, 4)), dict(precision=8), dict(recon=8),
+    for bad in [dict(dims=(4, 4, 3, 4)), dict(dims=(2, 4, 4, 4)), dict(precision=8), dict(recon=10),
                 dict(bc=(1, 1, 1, 0.5))]:
         kw = dict(dims=(4, 4, 4, 4), precision=64, recon=18, bc=(1, 1, 1, -1))
         kw.update(bad)

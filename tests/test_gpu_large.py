@@ -38,20 +38,24 @@ def cfg4():
     return c, U, psi
 
 
+@pytest.mark.parametrize("recon", [12, 8])
 @pytest.mark.parametrize("precision", [32, 64])
-def test_config4_eo_recon12_sampled(cfg4, precision):
+def test_config4_eo_recon12_sampled(cfg4, precision, recon):
     import gpu_harness as H
     c, U64, psi64 = cfg4
     dims, bc = c["dims"], c["bc"]
     U = U64.astype(H.cdtype(precision))
     psi = psi64.astype(H.cdtype(precision))
-    g = H.Gpu(dims, precision, 12, bc, U)
+    g = H.Gpu(dims, precision, recon, bc, U)
+    site_tol = H.site_tol_for(U, precision, recon)   # recon 8: from the conditioning of the worst of the 8.4 M links
     for out_parity in (0, 1):
         got = g.dslash_eo(H.half_of(psi, dims, 1 - out_parity), out_parity)
         sites = sample_sites(dims, out_parity, 4096, seed=40 + out_parity)
         ref = oracle.dslash_sites(U, psi, dims, bc, sites)
-        H.assert_parity(got[cb_index(dims, sites)], ref, precision)
+        H.assert_parity(got[cb_index(dims, sites)], ref, precision, site_tol=site_tol)
         assert np.isfinite(got.view(np.float32 if precision == 32 else np.float64)).all()
+    if recon != 12:
+        return
     # host-buffer entry point (what bench.py's e2e leg times) gives the same result bit for bit
     import torch
     ws = torch.empty(g.ctx.host_workspace_bytes(), dtype=torch.uint8, device="cuda:0")

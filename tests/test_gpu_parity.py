@@ -58,20 +58,21 @@ def test_config1_free_field_plane_wave(H):
 
 
 # ------------------------------------------------------------------ config 2: 8^3x16 fp64 eo
-@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("recon", [18, 12, 8])
 def test_config2_eo_fp64(H, recon):
     c, U, psi = _inputs(2, 64)
     dims, bc = c["dims"], c["bc"]
     g = H.Gpu(dims, 64, recon, bc, U)
+    st = H.site_tol_for(U, 64, recon)
     for out_parity in (0, 1):
         ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, out_parity), dims, out_parity)
         got = g.dslash_eo(H.half_of(psi, dims, 1 - out_parity), out_parity)
-        H.assert_parity(got, ref, 64)
+        H.assert_parity(got, ref, 64, site_tol=st)
     # even-odd pieces reassemble the full operator (pin P4 on the GPU)
     full = g.dslash_full(psi)
-    H.assert_parity(full, oracle.dslash_full(U, psi, dims, bc), 64)
+    H.assert_parity(full, oracle.dslash_full(U, psi, dims, bc), 64, site_tol=st)
     refM = H.half_of(oracle.apply_M(U, psi, dims, bc, c["kappa"], 1), dims, 0)
-    H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), c["kappa"], 1), refM, 64)
+    H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), c["kappa"], 1), refM, 64, site_tol=st)
 
 
 def test_config2_gamma5_hermiticity_and_covariance(H):
@@ -96,19 +97,20 @@ def test_config2_gamma5_hermiticity_and_covariance(H):
 
 
 # ------------------------------------------------------------------ config 3: 16^3x32 full, fp32 + fp64
-@pytest.mark.parametrize("precision,recon", [(64, 18), (64, 12), (32, 18), (32, 12)])
+@pytest.mark.parametrize("precision,recon", [(64, 18), (64, 12), (32, 18), (32, 12), (64, 8), (32, 8)])
 def test_config3_full(H, precision, recon):
     c, U, psi = _inputs(3, precision)
     dims, bc = c["dims"], c["bc"]
     g = H.Gpu(dims, precision, recon, bc, U)
-    H.assert_parity(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc), precision)
+    st = H.site_tol_for(U, precision, recon)
+    H.assert_parity(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc), precision, site_tol=st)
     refM = oracle.apply_M(U, psi, dims, bc, c["kappa"], 0)
-    H.assert_parity(g.apply_M(psi, c["kappa"], 0), refM, precision)
+    H.assert_parity(g.apply_M(psi, c["kappa"], 0), refM, precision, site_tol=st)
 
 
 # ------------------------------------------------------------------ edge cases
 @pytest.mark.parametrize("precision", [64, 32])
-@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("recon", [18, 12, 8])
 def test_ragged_anisotropic_complex_bc(H, precision, recon):
     """Vh = 960 is not a multiple of the block size; all extents differ; general U(1) phases."""
     from gpu_harness import cdtype
@@ -117,12 +119,13 @@ def test_ragged_anisotropic_complex_bc(H, precision, recon):
     U = li.random_su3_links(dims, seed=21).astype(cdtype(precision))
     psi = li.gaussian_spinor(dims, seed=22).astype(cdtype(precision))
     g = H.Gpu(dims, precision, recon, bc, U)
-    H.assert_parity(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc), precision)
+    st = H.site_tol_for(U, precision, recon)
+    H.assert_parity(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc), precision, site_tol=st)
     for op in (0, 1):
         ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, op), dims, op)
-        H.assert_parity(g.dslash_eo(H.half_of(psi, dims, 1 - op), op), ref, precision)
+        H.assert_parity(g.dslash_eo(H.half_of(psi, dims, 1 - op), op), ref, precision, site_tol=st)
     refM = H.half_of(oracle.apply_M(U, psi, dims, bc, 0.13, 1), dims, 0)
-    H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), 0.13, 1), refM, precision)
+    H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), 0.13, 1), refM, precision, site_tol=st)
 
 
 @pytest.mark.parametrize("dims", [(6, 6, 6, 6), (4, 6, 6, 6), (6, 4, 6, 10)])
@@ -211,7 +214,7 @@ def test_error_codes(H):
 
 
 # ------------------------------------------------------------------ next row f1: twisted-mass matrix
-@pytest.mark.parametrize("precision,recon", [(64, 18), (64, 12), (32, 12), (32, 18)])
+@pytest.mark.parametrize("precision,recon", [(64, 18), (64, 12), (32, 12), (32, 18), (64, 8), (32, 8)])
 def test_twisted_mass_matrix(H, precision, recon):
     """lqcd_apply_M_tm against oracle.apply_M_tm: full and even-odd (Schur complement) form, both signs of mu,
     on configs 2 (random SU(3)) and the ragged anisotropic lattice with complex boundary phases."""
@@ -222,11 +225,12 @@ def test_twisted_mass_matrix(H, precision, recon):
     for dims, bc, U, psi, kappa in cases:
         U, psi = U.astype(cdtype(precision)), psi.astype(cdtype(precision))
         g = H.Gpu(dims, precision, recon, bc, U)
+        st = H.site_tol_for(U, precision, recon)
         for mu in (0.25, -0.4):
             ref = oracle.apply_M_tm(U, psi, dims, bc, kappa, mu, 0)
-            H.assert_parity(g.apply_M(psi, kappa, 0, mu=mu), ref, precision)
+            H.assert_parity(g.apply_M(psi, kappa, 0, mu=mu), ref, precision, site_tol=st)
             ref = H.half_of(oracle.apply_M_tm(U, psi, dims, bc, kappa, mu, 1), dims, 0)
-            H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), kappa, 1, mu=mu), ref, precision)
+            H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), kappa, 1, mu=mu), ref, precision, site_tol=st)
         # mu = 0 is lqcd_apply_M bit for bit
         a = g.apply_M(H.half_of(psi, dims, 0), kappa, 1, mu=0.0)
         b = g.apply_M(H.half_of(psi, dims, 0), kappa, 1)
@@ -372,4 +376,48 @@ def test_fp32_spinors_with_half_links(H):
     import paper_1112_5280_b200 as L
     with pytest.raises(L.LqcdError) as e:
         L.Context(dims, 64, 12, bc, 16)
+    assert e.value.status == L.LQCD_EUNSUPPORTED
+
+
+# ------------------------------------------------------------------ next row f4: 8-real link storage
+@pytest.mark.parametrize("precision", [64, 32])
+def test_recon8_links(H, precision):
+    """lqcd_pack_gauge with recon = 8: the stored reals are the oracle's pack8 (phases to rounding), the margin the
+    library reports is the numpy one, and the operator matches the oracle fed the full 18-real links at north_star's
+    rel-L2 tolerances; the per-site bar follows the conditioning of the worst link."""
+    import torch
+    from oracle import recon8_oracle as r8
+    cd = H.cdtype(precision)
+    for dims, U in (((8, 8, 8, 16), li.links_for_config(2)), ((6, 6, 6, 6), li.near_unit_links((6, 6, 6, 6), seed=5, eps=0.3))):
+        U = U.astype(cd)
+        bc = (1, 1, 1, -1)
+        psi = li.gaussian_spinor(dims, seed=33).astype(cd)
+        g = H.Gpu(dims, precision, 8, bc, U)
+        assert g.ctx.gauge_bytes() == 2 * 8 * 8 * 32 * ((g.ctx.Vh + 31) // 32) * (precision // 8)
+        site_tol, margin = H.site_tol_for(U, precision, 8), H.recon8_margin(U)
+        scratch = torch.zeros(1, dtype=torch.float64, device="cuda:0")
+        got_margin = g.ctx.gauge_recon8_margin(torch.from_numpy(np.ascontiguousarray(U)).to("cuda:0"), scratch)
+        assert abs(got_margin - margin) <= 1e-6 * margin
+        # the packed reals: forward link of the even site cb = 0 is hop 0 of tile 0, lane 0: words [hop][w 2][32][4]
+        real = torch.float64 if precision == 64 else torch.float32
+        nat = g.gauge.view(real).cpu().numpy().reshape(2, -1, 8, 2, 32, 4)
+        for mu in range(4):
+            stored = nat[0, 0, 2 * mu, :, 0, :].reshape(8)
+            want = r8.pack8(U[mu, 0, 0, 0, 0])
+            d = stored - want
+            d[6:] = (d[6:] + 1.0) % 2.0 - 1.0
+            assert np.abs(d).max() <= (1e-15 if precision == 64 else 1e-7)
+        for op in (0, 1):
+            ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, op), dims, op)
+            H.assert_parity(g.dslash_eo(H.half_of(psi, dims, 1 - op), op), ref, precision, site_tol=site_tol)
+        H.assert_parity(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc), precision, site_tol=site_tol)
+        refM = H.half_of(oracle.apply_M_tm(U, psi, dims, bc, 0.15, 0.3, 1), dims, 0)
+        H.assert_parity(g.apply_M(H.half_of(psi, dims, 0), 0.15, 1, mu=0.3), refM, precision, site_tol=site_tol)
+    # unit links are outside the encoding: the library says so (margin 0) and precision 16 has no 8-real variant
+    dims = (4, 4, 4, 4)
+    c = H.Gpu(dims, precision, 8, (1, 1, 1, -1), li.random_su3_links(dims, seed=3).astype(cd)).ctx
+    assert c.gauge_recon8_margin(torch.from_numpy(li.unit_links(dims).astype(cd)).to("cuda:0"), scratch) == 0.0
+    import paper_1112_5280_b200 as L
+    with pytest.raises(L.LqcdError) as e:
+        L.Context(dims, 16, 8)
     assert e.value.status == L.LQCD_EUNSUPPORTED
