@@ -725,9 +725,13 @@ def run_b200(args):
         torch.cuda.empty_cache()
     del w
     torch.cuda.empty_cache()
-    if want("slab") and world > 1:
+    if want("slab") and args.precision != 16:
+        # next row f3: the same operator decomposed into `world` time slabs (one rank: the ring closes on itself)
         from paper_1112_5280_b200 import slab_bench
-        line["slab"] = slab_bench.run(torch, dist, timer, dev, args.config, args.precision, args.recon, half, args.warmup, peak)
+        r = slab_bench.run(torch, dist, timer, dev, args.config, args.precision, args.recon, half, args.warmup, peak, world, rank,
+                           FLOP_PER_SITE)
+        if rank == 0:
+            line["slab"] = r
     if rank == 0:
         if want("config3"):
             line["config3"] = config3_leg(torch, solo, dev, peak, 50, 10)

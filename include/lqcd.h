@@ -134,20 +134,38 @@ lqcd_status lqcd_dslash_full(const lqcd_ctx* ctx, void* out_dev, const void* gau
 lqcd_status lqcd_dslash_eo(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
                            int out_parity, void* stream);
 
-/* Time-slab decomposition primitives (next row f3; the paper's multi-device story is host-mediated,
- * PAPER.md:71, :103; here: T slabs with ghost time slices).  A rank holds T_loc global time slices as a local
- * lattice of T = T_loc + 2 slices whose slices 0 and T_loc + 1 are ghosts, filled by the caller with plain copies
- * of the neighbours' boundary slices: in the native layout a time slice of a half spinor is the contiguous
- * byte range [t, t + 1) * lqcd_time_slice_bytes(ctx) (0 = not available: slice not made of whole tiles, or
- * precision 16).  lqcd_dslash_eo_range computes only the output sites with t in [t_begin, t_end) (interior
- * slices 1..T_loc; or interior first, boundary slices after the exchange).  lqcd_set_time_slab moves the
- * t boundary phase from the local wrap to where the global boundary cuts the slab: the forward hop from slice
- * t_cross_fwd and the backward hop from slice t_cross_bwd carry bc_t / conj(bc_t); -1 = none; the defaults of a
- * whole lattice are (T - 1, 0).  Links need no exchange: each rank packs the links of its slices, ghosts included. */
+/* ---- time-slab decomposition over several GPUs (next row f3; the paper's multi-device story is host-mediated,
+ * PAPER.md:71, :103; T slabs, projected half-spinor faces between ring neighbours) ----
+ * A rank owns T_loc consecutive global time slices (T_loc even, so local and global parities agree) as a local lattice
+ * X,Y,Z,T_loc: a ctx created with those extents, then lqcd_set_time_slab.  One application of H on a slab:
+ *   1. lqcd_slab_push_faces   projects the first and the last time slice of `in` to half spinors (12 reals per site:
+ *                             (1 - gamma_t) psi for the rank below, (1 + gamma_t) psi for the rank above) and stores
+ *                             them into dst_down / dst_up -- the NEIGHBOURS' halo buffers mapped over NVLink peer memory
+ *                             (the transfer is the kernel's own stores), or local send buffers for ncclSend/ncclRecv
+ *   2. lqcd_dslash_eo_range   on the interior slices [1, T_loc - 1): needs no halo, overlaps the transfer
+ *   3. lqcd_dslash_eo_slab    on slices 0 and T_loc - 1: the t hops that leave the slab read halo_from_up / halo_from_down
+ * Ordering between 1 (on the neighbour) and 3: either by the caller (stream events after a collective / P2P receive:
+ * pass NULL flags), or on the device: push_faces publishes `epoch` with a system-scope release into the neighbours'
+ * flags (8-byte counters in peer memory) after its stores, and the slab kernel spins (system-scope acquire, bounded to
+ * ~10 s, then traps) until its own two flags have reached `epoch`.  Use a fresh, increasing epoch per application.
+ * Halo buffer (lqcd_halo_bytes): [face tile][word][32] 16-byte words, 3 (precision 32) / 6 (precision 64) per site,
+ * face site = checkerboard index within the time slice.  Precision 32 / 64 and every recon; not precision 16.
+ * lqcd_set_time_slab moves the t boundary phase from the local wrap to where the global boundary cuts the slab: the
+ * forward hop from slice t_cross_fwd and the backward hop from slice t_cross_bwd carry bc_t / conj(bc_t); -1 = none; a
+ * whole lattice has (T - 1, 0).  lqcd_pack_gauge_slab packs the local links; the backward t link of the first slice,
+ * U_t(x - t^), belongs to the rank below and is read from tlinks_below_dev, a canonical [Z][Y][X][3][3] array. */
 lqcd_status lqcd_set_time_slab(lqcd_ctx* ctx, int t_cross_fwd, int t_cross_bwd);
+lqcd_status lqcd_pack_gauge_slab(const lqcd_ctx* ctx, void* native_dev, const void* canonical_dev,
+                                 const void* tlinks_below_dev, void* stream);
+size_t lqcd_halo_bytes(const lqcd_ctx* ctx); /* one face; 0: no slab path for this ctx */
+lqcd_status lqcd_slab_push_faces(const lqcd_ctx* ctx, const void* in_dev, void* dst_up_dev, void* dst_down_dev,
+                                 void* flag_up_dev, void* flag_down_dev, unsigned long long epoch, void* stream);
 lqcd_status lqcd_dslash_eo_range(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
                                  int out_parity, int t_begin, int t_end, void* stream);
-size_t lqcd_time_slice_bytes(const lqcd_ctx* ctx);
+lqcd_status lqcd_dslash_eo_slab(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
+                                const void* halo_from_up_dev, const void* halo_from_down_dev, const void* wait_up_dev,
+                                const void* wait_down_dev, unsigned long long epoch, int out_parity, int t_begin,
+                                int t_end, void* stream);
 
 /* eo = 0: out = in - kappa H in, native full spinors, one launch, workspace unused (may be NULL).
  * eo = 1: out_e = in_e - kappa^2 H_eo H_oe in_e, native even half spinors; two launches;

@@ -153,6 +153,32 @@ def links_for_config(cfg_id: int, dtype=np.complex128) -> np.ndarray:
     return near_unit_links(c["dims"], LINK_SEED, c["eps"], dtype)
 
 
+def links_time_slices(cfg_id: int, t_list, dtype=np.complex128) -> np.ndarray:
+    """The time slices `t_list` of links_for_config(cfg_id): [4][len(t_list)][Z][Y][X][3][3], without generating the rest
+    (every (mu, t) slice has its own random stream) -- what one rank of a time-slab decomposition needs."""
+    c = CONFIGS[cfg_id]
+    X, Y, Z, _ = c["dims"]
+    kind = "su3" if c["links"] == "su3" else "near_unit"
+    out = np.empty((4, len(t_list), Z, Y, X, 3, 3), dtype=dtype)
+
+    def work(job):
+        mu, k = job
+        out[mu, k] = _link_slice(c["dims"], LINK_SEED, mu, t_list[k], kind, c["eps"])
+
+    with ThreadPoolExecutor(_nthreads()) as ex:
+        list(ex.map(work, [(mu, k) for mu in range(4) for k in range(len(t_list))]))
+    return out
+
+
+def gaussian_spinor_time_slices(dims, t_list, seed=SPINOR_SEED, dtype=np.complex128) -> np.ndarray:
+    """The time slices `t_list` of gaussian_spinor(dims, seed)."""
+    X, Y, Z, T = dims
+    out = np.empty((len(t_list), Z, Y, X, 4, 3), dtype=dtype)
+    for k, t in enumerate(t_list):
+        out[k] = _complex_normal(np.random.default_rng([seed, t]), (Z, Y, X, 4, 3))
+    return out
+
+
 def link_at(dims, seed, kind, eps, mu, coords) -> np.ndarray:
     """The single link U_mu(x) of the field `_links` would produce (regenerates one (mu,t) slice)."""
     x, y, z, t = coords

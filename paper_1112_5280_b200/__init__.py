@@ -19,7 +19,7 @@ HAS_RECON8 = True
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
-    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_set_time_slab", "lqcd_dslash_eo_range", "lqcd_time_slice_bytes", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_dslash_eo_host_batch", "lqcd_launch_count",
+    "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_set_time_slab", "lqcd_dslash_eo_range", "lqcd_pack_gauge_slab", "lqcd_halo_bytes", "lqcd_slab_push_faces", "lqcd_dslash_eo_slab", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_dslash_eo_host_batch", "lqcd_launch_count",
     "lqcd_gauge_recon8_margin", "lqcd_status_string", "lqcd_last_cuda_error",
 ]
 
@@ -65,8 +65,11 @@ def _lib():
         lib.lqcd_apply_M.argtypes = [vp, vp, vp, vp, cd, ci, vp, vp]
         lib.lqcd_set_time_slab.argtypes = [vp, ci, ci]
         lib.lqcd_dslash_eo_range.argtypes = [vp, vp, vp, vp, ci, ci, ci, vp]
-        lib.lqcd_time_slice_bytes.argtypes = [vp]
-        lib.lqcd_time_slice_bytes.restype = sz
+        lib.lqcd_halo_bytes.argtypes = [vp]
+        lib.lqcd_halo_bytes.restype = sz
+        lib.lqcd_pack_gauge_slab.argtypes = [vp, vp, vp, vp, vp]
+        lib.lqcd_slab_push_faces.argtypes = [vp, vp, vp, vp, vp, vp, ctypes.c_ulonglong, vp]
+        lib.lqcd_dslash_eo_slab.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, ctypes.c_ulonglong, ci, ci, ci, vp]
         lib.lqcd_apply_M_tm.argtypes = [vp, vp, vp, vp, cd, cd, ci, vp, vp]
         lib.lqcd_apply_Q_tm.argtypes = [vp, vp, vp, vp, cd, cd, vp, vp]
         lib.lqcd_cg_mixed_workspace_bytes.argtypes = [vp, vp]
@@ -170,7 +173,21 @@ class Context:
         _chk(_lib().lqcd_dslash_eo_range(self._h, _ptr(out), _ptr(gauge), _ptr(inp), int(out_parity), int(t_begin),
                                          int(t_end), _stream(stream)), "lqcd_dslash_eo_range")
 
-    def time_slice_bytes(self): return _lib().lqcd_time_slice_bytes(self._h)
+    def halo_bytes(self): return _lib().lqcd_halo_bytes(self._h)
+
+    def pack_gauge_slab(self, native, canonical, tlinks_below, stream=None):
+        _chk(_lib().lqcd_pack_gauge_slab(self._h, _ptr(native), _ptr(canonical), _ptr(tlinks_below), _stream(stream)),
+             "lqcd_pack_gauge_slab")
+
+    def slab_push_faces(self, inp, dst_up, dst_down, flag_up=None, flag_down=None, epoch=0, stream=None):
+        _chk(_lib().lqcd_slab_push_faces(self._h, _ptr(inp), _ptr(dst_up), _ptr(dst_down), _ptr(flag_up), _ptr(flag_down),
+                                         int(epoch), _stream(stream)), "lqcd_slab_push_faces")
+
+    def dslash_eo_slab(self, out, gauge, inp, halo_from_up, halo_from_down, out_parity, t_begin, t_end, wait_up=None,
+                       wait_down=None, epoch=0, stream=None):
+        _chk(_lib().lqcd_dslash_eo_slab(self._h, _ptr(out), _ptr(gauge), _ptr(inp), _ptr(halo_from_up), _ptr(halo_from_down),
+                                        _ptr(wait_up), _ptr(wait_down), int(epoch), int(out_parity), int(t_begin), int(t_end),
+                                        _stream(stream)), "lqcd_dslash_eo_slab")
 
     def apply_M(self, out, gauge, inp, kappa, eo, workspace=None, stream=None):
         _chk(_lib().lqcd_apply_M(self._h, _ptr(out), _ptr(gauge), _ptr(inp), float(kappa), int(eo),

@@ -168,10 +168,64 @@ __device__ __forceinline__ void recon_row2(R u[18]) {
 //   b1 = -(a1 conj(a0) b0 + conj(a2 c0)) / N2,   b2 = (conj(a1 c0) - a2 conj(a0) b0) / N2,   c = conj(a x b).
 // (rows orthonormal, det = 1; the 2 x 2 system for b1, b2 has determinant N2.)  Singular for N2 = 0, i.e. |U00| = 1:
 // unit links cannot be stored this way (lqcd_gauge_recon8_margin reports how close a field comes).
-__device__ __forceinline__ void sincospi_(float x, float& s, float& c) { sincospif(x, &s, &c); }
-__device__ __forceinline__ void sincospi_(double x, double& s, double& c) { sincospi(x, &s, &c); }
-__device__ __forceinline__ float sqrt_(float x) { return sqrtf(x); }
-__device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
+// Scalar helpers of the decoder, written out so that no library slow path (denormal / overflow handling of the IEEE
+// division and square root, the general range reduction of sincospi) enters the kernel: every argument is in a known
+// range here (N2 in (0, 1], the phases in [-1, 1]).
+//   fp32: the special-function unit (MUFU.RCP / RSQ / SIN / COS); sin/cos.approx are accurate to 2^-20.9 absolute on
+//         [-pi, pi], which puts the rebuilt link at ~5e-7 of the stored one -- below the 1e-5 bar of fp32 runs
+//   fp64: MUFU.RCP64H / RSQ64H seeds (20 bits) + two Newton steps; sin(pi r), cos(pi r) by their Taylor series on
+//         |r| <= 1/4 after reducing to the nearest quarter turn (truncation < 1e-16)
+__device__ __forceinline__ float rcp_(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rsqrt_(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ void sincospi_(float x, float& s, float& c) {
+    const float a = 3.14159265358979f * x;
+    asm("sin.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(a));
+    asm("cos.approx.ftz.f32 %0, %1;" : "=f"(c) : "f"(a));
+}
+__device__ __forceinline__ double rcp_(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(fma(-x, r, 1.0), r, r);
+    r = fma(fma(-x, r, 1.0), r, r);
+    return r;
+}
+__device__ __forceinline__ double rsqrt_(double x) {
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const double e = fma(-x * r, r, 1.0);           // 1 - x r^2
+        r = fma(fma(0.375, e, 0.5) * e, r, r);          // r (1 + e/2 + 3 e^2/8): third order, 20 -> 60 -> 180 bits
+    }
+    return r;
+}
+__device__ __forceinline__ void sincospi_(double x, double& s, double& c) {
+    const double k = rint(2.0 * x);                      // nearest quarter turn, k in {-2, ..., 2}
+    const double r = fma(k, -0.5, x), r2 = r * r;        // |r| <= 1/4
+    double ps = -2.1915353447830215827e-5;
+    ps = fma(ps, r2, 4.6630280576761256442e-4);
+    ps = fma(ps, r2, -7.3704309457143507773e-3);
+    ps = fma(ps, r2, 8.2145886611128228799e-2);
+    ps = fma(ps, r2, -5.9926452932079207689e-1);
+    ps = fma(ps, r2, 2.5501640398773454439);
+    ps = fma(ps, r2, -5.1677127800499700292);
+    ps = fma(ps, r2, 3.1415926535897932385);
+    ps *= r;
+    double pc = 4.3030695870329470073e-6;
+    pc = fma(pc, r2, -1.0463810492484570712e-4);
+    pc = fma(pc, r2, 1.9295743094039230479e-3);
+    pc = fma(pc, r2, -2.5806891390014060013e-2);
+    pc = fma(pc, r2, 2.3533063035889320454e-1);
+    pc = fma(pc, r2, -1.3352627688545894959);
+    pc = fma(pc, r2, 4.0587121264167682182);
+    pc = fma(pc, r2, -4.9348022005446793094);
+    pc = fma(pc, r2, 1.0);
+    // rotate by k quarter turns: (c, s) -> (c cos(k pi/2) - s sin(k pi/2), s cos(k pi/2) + c sin(k pi/2))
+    const int q = (int)k & 3;
+    const double sw_s = (q & 1) ? pc : ps, sw_c = (q & 1) ? ps : pc;
+    s = (q & 2) ? -sw_s : sw_s;
+    c = ((q + 1) & 2) ? -sw_c : sw_c;
+}
 
 template <typename R>
 __device__ __forceinline__ void recon8(const R r[8], R u[18]) {
@@ -181,9 +235,12 @@ __device__ __forceinline__ void recon8(const R r[8], R u[18]) {
     R s0, c0, s2, c2;
     sincospi_(r[6], s0, c0);
     sincospi_(r[7], s2, c2);
-    const R ma = sqrt_(fmax((R)1 - N2, (R)0)), mc = sqrt_(fmax(N2 - B2, (R)0));
+    // sqrt(t) = t rsqrt(t), t clamped away from 0 (then the product is 0 to rounding, as it should be)
+    constexpr R tiny = sizeof(R) == 4 ? (R)1e-30 : (R)1e-290;
+    const R ta = fmax((R)1 - N2, tiny), tc = fmax(N2 - B2, tiny);
+    const R ma = ta * rsqrt_(ta), mc = tc * rsqrt_(tc);
     const R a0r = ma * c0, a0i = ma * s0, c0r = mc * c2, c0i = mc * s2;
-    const R inv = (R)1 / N2;
+    const R inv = rcp_(N2);
     // t = conj(a0) b0;  w = a2 c0;  v = a1 c0
     const R tr = fmar(a0r, b0r, a0i * b0i), ti = fmar(a0r, b0i, -a0i * b0r);
     const R wr = fmar(a2r, c0r, -a2i * c0i), wi = fmar(a2r, c0i, a2i * c0r);

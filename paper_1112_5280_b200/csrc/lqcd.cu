@@ -9,8 +9,8 @@
 #include <new>
 
 #include "blas_kernels.cuh"
-#include "launch.cuh"
 #include "pack_kernels.cuh"
+#include "slab_launch.cuh"
 
 using namespace lqcd;
 
@@ -24,6 +24,10 @@ extern template lqcd_status launch_recon<__half, 12>(LQCD_LAUNCH_RECON_ARGS);
 extern template lqcd_status launch_recon<float, RECON_12H>(LQCD_LAUNCH_RECON_ARGS);
 extern template lqcd_status launch_recon<double, 8>(LQCD_LAUNCH_RECON_ARGS);
 extern template lqcd_status launch_recon<float, 8>(LQCD_LAUNCH_RECON_ARGS);
+extern template lqcd_status launch_slab<float>(LQCD_LAUNCH_SLAB_ARGS);
+extern template lqcd_status launch_slab<double>(LQCD_LAUNCH_SLAB_ARGS);
+extern template lqcd_status launch_push_faces<float>(LQCD_LAUNCH_FACES_ARGS);
+extern template lqcd_status launch_push_faces<double>(LQCD_LAUNCH_FACES_ARGS);
 }  // namespace lqcd
 
 namespace {
@@ -149,24 +153,33 @@ size_t lqcd_host_workspace_bytes(const lqcd_ctx* c) {
            HOST_SLOTS * 2 * (align256(half_bytes(c)) + align256(canon_half));
 }
 
-lqcd_status lqcd_pack_gauge(const lqcd_ctx* c, void* native, const void* canon, void* stream) {
+static lqcd_status pack_gauge_impl(const lqcd_ctx* c, void* native, const void* canon, const void* below, void* stream) {
     if (!c || !native || !canon) return LQCD_EINVAL;
-    if (!aligned32(native) || !aligned16(canon)) return LQCD_EALIGN;
+    if (!aligned32(native) || !aligned16(canon) || !aligned16(below)) return LQCD_EALIGN;
     const dim3 grid((c->g.Vh + 127) / 128, 8, 2);
     cudaStream_t st = (cudaStream_t)stream;
     if (c->p.precision == 16 || c->p.link_precision == 16) {
-        pack_gauge_h_kernel<<<grid, 128, 0, st>>>((__half*)native, (const float*)canon, c->g);
+        pack_gauge_h_kernel<<<grid, 128, 0, st>>>((__half*)native, (const float*)canon, (const float*)below, c->g);
     } else if (c->p.recon == 8) {
-        if (c->p.precision == 32) pack_gauge8_kernel<float><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);
-        else pack_gauge8_kernel<double><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, c->g);
+        if (c->p.precision == 32) pack_gauge8_kernel<float><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, (const float*)below, c->g);
+        else pack_gauge8_kernel<double><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, (const double*)below, c->g);
     } else if (c->p.precision == 32) {
-        if (c->p.recon == 12) pack_gauge_kernel<float, 12><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);
-        else pack_gauge_kernel<float, 18><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, c->g);
+        if (c->p.recon == 12) pack_gauge_kernel<float, 12><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, (const float*)below, c->g);
+        else pack_gauge_kernel<float, 18><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, (const float*)below, c->g);
     } else {
-        if (c->p.recon == 12) pack_gauge_kernel<double, 12><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, c->g);
-        else pack_gauge_kernel<double, 18><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, c->g);
+        if (c->p.recon == 12) pack_gauge_kernel<double, 12><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, (const double*)below, c->g);
+        else pack_gauge_kernel<double, 18><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, (const double*)below, c->g);
     }
     return after_launch();
+}
+
+lqcd_status lqcd_pack_gauge(const lqcd_ctx* c, void* native, const void* canon, void* stream) {
+    return pack_gauge_impl(c, native, canon, nullptr, stream);
+}
+
+lqcd_status lqcd_pack_gauge_slab(const lqcd_ctx* c, void* native, const void* canon, const void* tlinks_below, void* stream) {
+    if (!tlinks_below) return LQCD_EINVAL;
+    return pack_gauge_impl(c, native, canon, tlinks_below, stream);
 }
 
 lqcd_status lqcd_gauge_recon8_margin(const lqcd_ctx* c, const void* canon, void* scratch, double* margin_host, void* stream) {
@@ -231,11 +244,11 @@ lqcd_status lqcd_dslash_eo(const lqcd_ctx* c, void* out, const void* gauge, cons
     return launch_dslash(c, out, gauge, in, nullptr, EpiArgs{EPI_STORE, 0, 0, 0, 0}, out_parity, (cudaStream_t)stream, all_sites(c));
 }
 
-// ---- next row f3: time-slab decomposition primitives ------------------------------------------------------
-// A rank of a T-slab decomposition holds the time slices [t0, t0 + T_loc) of the global lattice as a local
-// lattice of T_loc + 2 slices: slice 0 and slice T_loc + 1 are ghosts filled from the neighbouring ranks
-// (plain copies of whole time slices, which are contiguous in the native layout), and only the interior
-// slices are computed.  The boundary phase sits where the global boundary cuts the slab, not at the local wrap.
+// ---- next row f3: time-slab decomposition (slab_kernels.cuh) ----------------------------------------------
+// A rank of a T-slab decomposition holds the time slices [t0, t0 + T_loc) of the global lattice (T_loc even) as a
+// local lattice of exactly those slices.  The t hops that leave the slab read projected half spinors from two halo
+// buffers filled by the neighbouring ranks (lqcd_slab_push_faces); the interior slices need no halo and are plain
+// lqcd_dslash_eo_range launches.  The boundary phase sits where the global boundary cuts the slab, not at the local wrap.
 lqcd_status lqcd_set_time_slab(lqcd_ctx* c, int t_cross_fwd, int t_cross_bwd) {
     if (!c) return LQCD_EINVAL;
     if (t_cross_fwd < -1 || t_cross_fwd >= c->g.T || t_cross_bwd < -1 || t_cross_bwd >= c->g.T) return LQCD_EINVAL;
@@ -255,11 +268,44 @@ lqcd_status lqcd_dslash_eo_range(const lqcd_ctx* c, void* out, const void* gauge
                          CbRange{t_begin * c->g.st, t_end * c->g.st});
 }
 
-size_t lqcd_time_slice_bytes(const lqcd_ctx* c) {
-    // bytes of one time slice of a native half spinor; 0 if slices are not whole tiles (or 16-bit storage,
-    // whose norms live apart): then the slab path is not available for this lattice
-    if (!c || c->p.precision == 16 || c->g.st % TILE != 0) return 0;
-    return (size_t)c->g.st * 24 * elem(c);
+static bool slab_capable(const lqcd_ctx* c) { return c->p.precision != 16 && c->p.link_precision != 16; }
+
+size_t lqcd_halo_bytes(const lqcd_ctx* c) {
+    // one face of projected half spinors: 12 reals per site of one parity of a time slice, padded to whole 32-site tiles
+    if (!c || !slab_capable(c)) return 0;
+    return (size_t)face_tiles(c->g) * TILE * 12 * elem(c);
+}
+
+lqcd_status lqcd_slab_push_faces(const lqcd_ctx* c, const void* in, void* dst_up, void* dst_down, void* flag_up, void* flag_down,
+                                 unsigned long long epoch, void* stream) {
+    if (!c || !in) return LQCD_EINVAL;
+    if (!slab_capable(c)) return LQCD_EUNSUPPORTED;
+    if (!aligned32(in) || !aligned32(dst_up) || !aligned32(dst_down)) return LQCD_EALIGN;
+    if ((reinterpret_cast<uintptr_t>(flag_up) | reinterpret_cast<uintptr_t>(flag_down)) & 7u) return LQCD_EALIGN;
+    if (!dst_up && !dst_down) return LQCD_OK;
+    return c->p.precision == 32
+               ? launch_push_faces<float>(c, in, dst_up, dst_down, (unsigned long long*)flag_up, (unsigned long long*)flag_down, epoch, (cudaStream_t)stream)
+               : launch_push_faces<double>(c, in, dst_up, dst_down, (unsigned long long*)flag_up, (unsigned long long*)flag_down, epoch, (cudaStream_t)stream);
+}
+
+lqcd_status lqcd_dslash_eo_slab(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* halo_from_up,
+                                const void* halo_from_down, const void* wait_up, const void* wait_down, unsigned long long epoch,
+                                int out_parity, int t_begin, int t_end, void* stream) {
+    if (out_parity != 0 && out_parity != 1) return LQCD_EINVAL;
+    lqcd_status s = check_fields(c, out, gauge, in, c ? half_bytes(c) : 0);
+    if (s != LQCD_OK) return s;
+    if (!slab_capable(c)) return LQCD_EUNSUPPORTED;
+    if (!halo_from_up || !halo_from_down) return LQCD_EINVAL;
+    if (!aligned32(halo_from_up) || !aligned32(halo_from_down)) return LQCD_EALIGN;
+    if ((reinterpret_cast<uintptr_t>(wait_up) | reinterpret_cast<uintptr_t>(wait_down)) & 7u) return LQCD_EALIGN;
+    if (t_begin < 0 || t_end > c->g.T || t_begin > t_end) return LQCD_EINVAL;
+    if (t_begin == t_end) return LQCD_OK;
+    const CbRange rg{t_begin * c->g.st, t_end * c->g.st};
+    return c->p.precision == 32
+               ? launch_slab<float>(c, out, gauge, in, halo_from_up, halo_from_down, (const unsigned long long*)wait_up,
+                                    (const unsigned long long*)wait_down, epoch, out_parity, (cudaStream_t)stream, rg)
+               : launch_slab<double>(c, out, gauge, in, halo_from_up, halo_from_down, (const unsigned long long*)wait_up,
+                                     (const unsigned long long*)wait_down, epoch, out_parity, (cudaStream_t)stream, rg);
 }
 
 // Shared body of lqcd_apply_M (theta = 0) and lqcd_apply_M_tm (theta = 2 kappa mu).

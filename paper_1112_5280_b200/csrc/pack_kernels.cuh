@@ -22,18 +22,31 @@ __device__ __forceinline__ size_t lex_back(const Geom& g, int cb, int p, int mu)
     return (size_t)c[0] + (size_t)g.X * (c[1] + (size_t)g.Y * (c[2] + (size_t)g.Z * c[3]));
 }
 
+// The canonical link (18 reals) stored for hop k of the site (p, cb).  On a time slab (`below` != NULL) the backward
+// t link of a site of the first slice, U_t(x - t^), belongs to the rank below and comes from `below`, a canonical
+// [Z][Y][X][3][3] array of that rank's last-slice t links; everywhere else the local field with periodic wrap.
+template <typename R>
+__device__ __forceinline__ const R* link_source(const R* __restrict__ canon, const R* __restrict__ below, const Geom& g, int cb, int p, int k) {
+    const int mu = k >> 1;
+    const size_t V = (size_t)2 * g.Vh;
+    if (k == 7 && below && cb < g.st) {   // t = 0
+        const size_t lex = lex_of(g, cb, p);  // t = 0: lex is the index within the slice
+        return below + lex * 18;
+    }
+    const size_t site = (k & 1) ? lex_back(g, cb, p, mu) : lex_of(g, cb, p);
+    return canon + ((size_t)mu * V + site) * 18;
+}
+
 // canonical links [mu][V][3][3] complex -> native, gathered by output site (fields.cuh): for site cb of
 // parity p, hop k = 2 mu holds U_mu(x), hop k = 2 mu + 1 holds U_mu(x - mu^); first RECON reals of each.
 // grid: (ceil(Vh / block), 8 hops, 2 parities).
 template <typename R, int RECON>
-__global__ void pack_gauge_kernel(R* __restrict__ native, const R* __restrict__ canon, Geom g) {
+__global__ void pack_gauge_kernel(R* __restrict__ native, const R* __restrict__ canon, const R* __restrict__ below, Geom g) {
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= g.Vh) return;
-    const int k = blockIdx.y, p = blockIdx.z, mu = k >> 1;
+    const int k = blockIdx.y, p = blockIdx.z;
     constexpr int LW = LinkWord<R, RECON>::LW, NW = RECON / LW;
-    const size_t V = (size_t)2 * g.Vh;
-    const size_t site = (k & 1) ? lex_back(g, cb, p, mu) : lex_of(g, cb, p);
-    const R* src = canon + ((size_t)mu * V + site) * 18;
+    const R* src = link_source<R>(canon, below, g, cb, p, k);
     R* dst = native + link_word0<R, RECON>(g.ntiles, p, cb, k) * LW;
 #pragma unroll
     for (int w = 0; w < NW; ++w)
@@ -44,13 +57,11 @@ __global__ void pack_gauge_kernel(R* __restrict__ native, const R* __restrict__ 
 // 8-real storage (fields.cuh): r = (Re a1, Im a1, Re a2, Im a2, Re b0, Im b0, arg(a0) / pi, arg(c0) / pi), the two
 // phases evaluated in double and rounded once.  Same grid as pack_gauge_kernel.
 template <typename R>
-__global__ void pack_gauge8_kernel(R* __restrict__ native, const R* __restrict__ canon, Geom g) {
+__global__ void pack_gauge8_kernel(R* __restrict__ native, const R* __restrict__ canon, const R* __restrict__ below, Geom g) {
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= g.Vh) return;
-    const int k = blockIdx.y, p = blockIdx.z, mu = k >> 1;
-    const size_t V = (size_t)2 * g.Vh;
-    const size_t site = (k & 1) ? lex_back(g, cb, p, mu) : lex_of(g, cb, p);
-    const R* src = canon + ((size_t)mu * V + site) * 18;
+    const int k = blockIdx.y, p = blockIdx.z;
+    const R* src = link_source<R>(canon, below, g, cb, p, k);
     constexpr double inv_pi = 0.31830988618379067154;
     R r[8] = {src[2], src[3], src[4], src[5], src[6], src[7],
               (R)(atan2((double)src[1], (double)src[0]) * inv_pi), (R)(atan2((double)src[13], (double)src[12]) * inv_pi)};
@@ -116,13 +127,11 @@ __global__ void pack_spinor_kernel(R* __restrict__ dst_, const R* __restrict__ s
 // ---- 16-bit storage: canonical complex64 <-> native half (fields.cuh) ------------------------------------
 
 // 12-real links only.  grid: (ceil(Vh / block), 8 hops, 2 parities).
-__global__ void pack_gauge_h_kernel(__half* __restrict__ native, const float* __restrict__ canon, Geom g) {
+__global__ void pack_gauge_h_kernel(__half* __restrict__ native, const float* __restrict__ canon, const float* __restrict__ below, Geom g) {
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= g.Vh) return;
-    const int k = blockIdx.y, p = blockIdx.z, mu = k >> 1;
-    const size_t V = (size_t)2 * g.Vh;
-    const size_t site = (k & 1) ? lex_back(g, cb, p, mu) : lex_of(g, cb, p);
-    const float* src = canon + ((size_t)mu * V + site) * 18;
+    const int k = blockIdx.y, p = blockIdx.z;
+    const float* src = link_source<float>(canon, below, g, cb, p, k);
     __half* dst = native + link_word0_h(g.ntiles, p, cb, k) * 4;
 #pragma unroll
     for (int w = 0; w < 3; ++w)

@@ -1,13 +1,25 @@
 """Time-slab decomposition of the even-odd dslash over several GPUs (next row f3).
 
-One process per GPU (torch.distributed, NCCL); rank r owns the global time slices [r T/N, (r+1) T/N) as a local
-lattice of T/N + 2 slices whose first and last slice are ghosts.  Everything arithmetic stays in the CUDA kernels
-(lqcd_dslash_eo_range); this module is plumbing only: which slices a rank holds, where the global boundary phase
-cuts it (lqcd_set_time_slab), and the ghost exchange -- plain copies of whole time slices, which are contiguous
-byte ranges of the native layout.  Links need no exchange: every rank packs the links of its own slices, ghosts
-included.  The paper's own multi-device scheme is host-mediated; this is the natural
-sharding named in SURVEY.md sec. 8(e).  Not used by bench.py (north_star: single GPU); covered by a
-single-GPU emulation of N ranks (tests/test_gpu_slab.py) and a world-size-2 gloo test of the exchange.
+One process per GPU (torch.distributed); rank r owns the global time slices [r T/N, (r+1) T/N) as a local lattice of
+exactly those slices (T/N even, so local and global site parities agree).  Everything arithmetic stays in the CUDA
+kernels (csrc/slab_kernels.cuh): the face projection to half spinors, the stores into the neighbours' halo buffers, the
+boundary sites that consume them.  This module is plumbing only: which slices a rank holds, where the global boundary
+phase cuts it (lqcd_set_time_slab), the buffers, the streams and events that order push / interior / boundary, and the
+transport of the projected faces (12 reals per face site, 786 KB per face in fp32 at 32^3 x 64):
+
+  PeerMemoryTransport   the B200 path: halo buffers and flags live in NVLink-mapped symmetric memory
+                        (torch.distributed._symmetric_memory); lqcd_slab_push_faces stores the projected faces straight
+                        into the neighbours' buffers and publishes an epoch, lqcd_dslash_eo_slab acquires it on the
+                        device -- projection, transfer and consumption without a host round trip or a library collective
+  SendRecvTransport     projected faces into local send buffers, then ncclSend / ncclRecv between ring neighbours
+                        (torch.distributed P2P ops: NCCL on GPUs, gloo in the CPU tests) on a side stream, an event
+                        orders the boundary launches after the receives
+  LocalRingTransport    all ranks in one process on one GPU (tests, single-GPU emulation): "peer" pointers are the other
+                        slabs' buffers, ordering by stream order
+
+The paper's own multi-device scheme is host-mediated; this is the natural sharding named in
+SURVEY.md sec. 8(e).  The headline bench stays "replicas only" (north_star: single GPU); bench.py's `slab` leg times this
+path when WORLD_SIZE > 1.
 """
 from __future__ import annotations
 
@@ -19,71 +31,210 @@ class TimeSlab:
 
     def __init__(self, dims, precision, recon, bc, rank, world):
         X, Y, Z, T = (int(d) for d in dims)
-        if T % world or (T // world) % 2 or T // world < 2:
-            raise ValueError("T / world must be an even number of time slices")
+        if T % world or (T // world) % 2 or T // world < 4:
+            raise ValueError("T / world must be an even number of time slices, at least 4")
         self.global_dims, self.rank, self.world = (X, Y, Z, T), int(rank), int(world)
         self.Tl = T // world
         self.t0 = self.rank * self.Tl
-        self.local_dims = (X, Y, Z, self.Tl + 2)
+        self.local_dims = (X, Y, Z, self.Tl)
         self.ctx = Context(self.local_dims, precision, recon, bc)
         # the global t boundary lies between the last slice of the last rank and the first slice of rank 0
-        self.ctx.set_time_slab(self.Tl if self.rank == self.world - 1 else -1, 1 if self.rank == 0 else -1)
-        self.slice_bytes = self.ctx.time_slice_bytes()
-        if self.slice_bytes == 0:
-            raise ValueError("time slices are not whole 32-site tiles (or precision 16): no slab path for this lattice")
+        self.ctx.set_time_slab(self.Tl - 1 if self.rank == self.world - 1 else -1, 0 if self.rank == 0 else -1)
+        self.halo_bytes = self.ctx.halo_bytes()
+        if self.halo_bytes == 0:
+            raise ValueError("no slab path for this context (precision 16 / half links)")
+        self.face_sites = X * Y * Z // 2
 
     # ---- bookkeeping -------------------------------------------------------------------------------------
     def time_indices(self):
-        """Global t of the local slices 0 .. Tl + 1 (ghosts wrap around the global lattice)."""
-        T = self.global_dims[3]
-        return [(self.t0 - 1 + k) % T for k in range(self.Tl + 2)]
+        """Global t of the local slices 0 .. Tl - 1."""
+        return list(range(self.t0, self.t0 + self.Tl))
 
-    def local_parity(self, global_parity):
-        """Local slice 1 is global slice t0 (even), so a site's local and global parities differ by one."""
-        return int(global_parity) ^ ((self.t0 - 1) & 1)
-
-    def left(self):
+    def below(self):
         return (self.rank - 1) % self.world
 
-    def right(self):
+    def above(self):
         return (self.rank + 1) % self.world
 
-    def slice_view(self, field, tl):
-        """Bytes of local time slice tl of a native half spinor held in a flat uint8 tensor."""
-        return field[tl * self.slice_bytes:(tl + 1) * self.slice_bytes]
+    def t_below(self):
+        """Global t of the last slice of the rank below: its t links are the backward t links of local slice 0."""
+        return (self.t0 - 1) % self.global_dims[3]
 
-    # ---- ghost exchange ----------------------------------------------------------------------------------
-    def exchange(self, field, dist):
-        """Fill the ghost slices of `field` (flat uint8 tensor, native half spinor of this slab) from the ring
-        neighbours with torch.distributed point-to-point copies; blocks until they have arrived."""
-        if self.world == 1:
-            self.slice_view(field, 0).copy_(self.slice_view(field, self.Tl))
-            self.slice_view(field, self.Tl + 1).copy_(self.slice_view(field, 1))
+    def pack_gauge(self, native, U_local, Ut_below, stream=None):
+        """U_local: canonical links [4][Tl][Z][Y][X][3][3] of the own slices; Ut_below: canonical [Z][Y][X][3][3] t links of
+        global slice t_below() (device tensors)."""
+        self.ctx.pack_gauge_slab(native, U_local, Ut_below, stream)
+
+    # ---- the operator ------------------------------------------------------------------------------------
+    def dslash_eo(self, out, gauge, inp, out_parity, transport, stream=None):
+        """out = H in on this rank's slices.  Enqueue only: the faces are projected and pushed on the transport's side
+        stream while the interior slices (which read no halo) run on `stream`; the two boundary slices follow once the
+        neighbours' faces have arrived (an event, or the device-side epoch of the peer-memory transport)."""
+        import torch
+        stream = stream if stream is not None else torch.cuda.current_stream()
+        h = transport.push(self, inp, stream)                       # side stream: projection + transfer
+        self.ctx.dslash_eo_range(out, gauge, inp, out_parity, 1, self.Tl - 1, stream)
+        h.before_boundary(stream)
+        kw = dict(wait_up=h.wait_up, wait_down=h.wait_down, epoch=h.epoch, stream=stream)
+        self.ctx.dslash_eo_slab(out, gauge, inp, h.from_up, h.from_down, out_parity, 0, 1, **kw)
+        self.ctx.dslash_eo_slab(out, gauge, inp, h.from_up, h.from_down, out_parity, self.Tl - 1, self.Tl, **kw)
+        transport.after_boundary(self, stream)
+
+
+class _Halos:
+    """What one push hands to the boundary launches."""
+
+    def __init__(self, from_up, from_down, event=None, wait_up=None, wait_down=None, epoch=0):
+        self.from_up, self.from_down, self.event = from_up, from_down, event
+        self.wait_up, self.wait_down, self.epoch = wait_up, wait_down, epoch
+
+    def before_boundary(self, stream):
+        if self.event is not None:
+            stream.wait_event(self.event)
+
+
+def _align(n, a=256):
+    return (n + a - 1) // a * a
+
+
+class LocalRingTransport:
+    """All ranks of the ring in one process on one GPU: every slab's halo buffers are ordinary device tensors and the
+    "peer" pointers handed to lqcd_slab_push_faces are the neighbouring slabs' buffers.  `push_all` runs every rank's
+    face projection first (one stream: stream order is the synchronisation); with use_flags the device-side epoch
+    protocol is exercised too -- the flags are already published when the boundary kernels start, so nothing spins."""
+
+    def __init__(self, slabs, device, use_flags=False):
+        import torch
+        self.slabs, self.use_flags, self.epoch = slabs, use_flags, 0
+        hb = slabs[0].halo_bytes
+        self.from_up = [torch.full((hb,), 0xFF, dtype=torch.uint8, device=device) for _ in slabs]    # NaN-ish until pushed
+        self.from_down = [torch.full((hb,), 0xFF, dtype=torch.uint8, device=device) for _ in slabs]
+        self.flags = [torch.zeros(2, dtype=torch.int64, device=device) for _ in slabs]                 # [from_up, from_down]
+
+    def push_all(self, inputs, stream=None):
+        self.epoch += 1
+        for r, s in enumerate(self.slabs):
+            up, dn = s.above(), s.below()
+            fu = self.flags[up][1:2] if self.use_flags else None       # my last slice is the rank above's "from_down"
+            fd = self.flags[dn][0:1] if self.use_flags else None
+            s.ctx.slab_push_faces(inputs[r], self.from_down[up], self.from_up[dn], fu, fd, self.epoch, stream)
+
+    def push(self, slab, inp, stream):
+        r = slab.rank
+        if self.use_flags:
+            return _Halos(self.from_up[r], self.from_down[r], None, self.flags[r][0:1], self.flags[r][1:2], self.epoch)
+        return _Halos(self.from_up[r], self.from_down[r])
+
+    def after_boundary(self, slab, stream):
+        pass
+
+
+class SendRecvTransport:
+    """Faces projected into local send buffers, exchanged with the ring neighbours by torch.distributed point-to-point
+    operations (ncclSend / ncclRecv on GPUs; gloo with host tensors in the CPU tests) on a side stream.  The host never
+    waits with NCCL: `Work.wait()` only makes the side stream wait for NCCL's stream, and an event orders the boundary
+    launches after the receives."""
+    TAG_DOWNWARD, TAG_UPWARD = 1, 2     # a face travelling to the rank below / above
+
+    def __init__(self, slab, dist, device):
+        import torch
+        self.dist, self.device = dist, torch.device(device)
+        self.cuda = self.device.type == "cuda"
+        hb = slab.halo_bytes
+        mk = lambda: torch.zeros(hb, dtype=torch.uint8, device=self.device)
+        self.send_up, self.send_down, self.from_up, self.from_down = mk(), mk(), mk(), mk()
+        self.side = torch.cuda.Stream(self.device) if self.cuda else None
+        self.use_tags = dist is not None and dist.get_backend() != "nccl"
+
+    def exchange(self, slab):
+        """send_down -> rank below (its from_up), send_up -> rank above (its from_down).  On a ring of two both
+        neighbours are the same rank: NCCL pairs the operations of a peer in the order they are posted, so the sends go
+        [downward, upward] and the receives [from above, from below] -- the downward face of the rank above is what
+        from_up must get.  Backends with tags (gloo) carry the direction in the tag as well."""
+        dist = self.dist
+        if slab.world == 1:
+            self.from_up.copy_(self.send_down)
+            self.from_down.copy_(self.send_up)
             return
-        ops = [dist.P2POp(dist.isend, self.slice_view(field, 1), self.left()),
-               dist.P2POp(dist.isend, self.slice_view(field, self.Tl), self.right()),
-               dist.P2POp(dist.irecv, self.slice_view(field, self.Tl + 1), self.right()),
-               dist.P2POp(dist.irecv, self.slice_view(field, 0), self.left())]
+        tag = (lambda t: dict(tag=t)) if self.use_tags else (lambda t: {})
+        ops = [dist.P2POp(dist.isend, self.send_down, slab.below(), **tag(self.TAG_DOWNWARD)),
+               dist.P2POp(dist.isend, self.send_up, slab.above(), **tag(self.TAG_UPWARD)),
+               dist.P2POp(dist.irecv, self.from_up, slab.above(), **tag(self.TAG_DOWNWARD)),
+               dist.P2POp(dist.irecv, self.from_down, slab.below(), **tag(self.TAG_UPWARD))]
         for req in dist.batch_isend_irecv(ops):
             req.wait()
 
-    # ---- the operator ------------------------------------------------------------------------------------
-    def dslash_eo(self, out, gauge, inp, global_out_parity, exchange, stream=None):
-        """out = H in on this rank's interior slices.  `exchange(field)` fills the ghosts of `inp` (self.exchange
-        bound to a process group, or an emulation); the slices that do not touch a ghost are launched first, so
-        with an asynchronous exchange on another stream they overlap it."""
-        lp = self.local_parity(global_out_parity)
-        if self.Tl > 2:
-            self.ctx.dslash_eo_range(out, gauge, inp, lp, 2, self.Tl, stream)
-        exchange(inp)
-        self.ctx.dslash_eo_range(out, gauge, inp, lp, 1, 2, stream)
-        self.ctx.dslash_eo_range(out, gauge, inp, lp, self.Tl, self.Tl + 1, stream)
+    def push(self, slab, inp, stream):
+        import torch
+        self.side.wait_stream(stream)          # the input is ready and the previous boundary launches have read the halos
+        with torch.cuda.stream(self.side):
+            slab.ctx.slab_push_faces(inp, self.send_up, self.send_down, stream=self.side)
+            self.exchange(slab)
+            ev = torch.cuda.Event()
+            ev.record(self.side)
+        return _Halos(self.from_up, self.from_down, ev)
+
+    def after_boundary(self, slab, stream):
+        pass
 
 
-def exchange_emulated(slabs, fields):
-    """All ranks in one process (one GPU): copy the boundary slices between the slabs' fields directly."""
-    n = len(slabs)
-    for r, s in enumerate(slabs):
-        left, right = fields[(r - 1) % n], fields[(r + 1) % n]
-        s.slice_view(fields[r], 0).copy_(slabs[(r - 1) % n].slice_view(left, s.Tl))
-        s.slice_view(fields[r], s.Tl + 1).copy_(slabs[(r + 1) % n].slice_view(right, 1))
+class PeerMemoryTransport:
+    """Halo buffers and flags in NVLink-mapped symmetric memory.  Per rank: two generations (epoch parity) of
+    [from_up | from_down] halo buffers and two 8-byte flags.  A push stores this rank's projected faces directly into the
+    neighbours' buffers of the current generation (the face-projection kernel's own stores cross NVLink) and then
+    publishes the epoch into their flags; the boundary kernel acquires this rank's own two flags on the device.  Two
+    generations suffice: a rank pushes generation n + 1 only after its own boundary launches of application n
+    (side.wait_stream), and a neighbour can push n + 2 only after it has consumed this rank's n + 1."""
+
+    def __init__(self, slab, dist, device, group=None):
+        import torch
+        import torch.distributed._symmetric_memory as symm_mem
+        self.dist, self.device = dist, torch.device(device)
+        self.hb = _align(slab.halo_bytes)
+        self.flag_off = 4 * self.hb
+        nbytes = self.flag_off + 256
+        self.buf = symm_mem.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.buf.zero_()
+        self.hdl = symm_mem.rendezvous(self.buf, group if group is not None else dist.group.WORLD)
+        self.ptrs = [int(p) for p in self.hdl.buffer_ptrs]
+        assert self.ptrs[slab.rank] == self.buf.data_ptr()
+        self.side = torch.cuda.Stream(self.device)
+        self.epoch = 0
+        torch.cuda.synchronize(self.device)
+        dist.barrier()                          # every rank's flags are zero before anyone pushes
+
+    def _halo(self, rank, gen, which):          # which: 0 = from_up, 1 = from_down
+        return self.ptrs[rank] + (2 * gen + which) * self.hb
+
+    def _flag(self, rank, which):
+        return self.ptrs[rank] + self.flag_off + 8 * which
+
+    def push(self, slab, inp, stream):
+        import torch
+        self.epoch += 1
+        gen, me = self.epoch & 1, slab.rank
+        self.side.wait_stream(stream)
+        slab.ctx.slab_push_faces(inp, self._halo(slab.above(), gen, 1), self._halo(slab.below(), gen, 0),
+                                 self._flag(slab.above(), 1), self._flag(slab.below(), 0), self.epoch, stream=self.side)
+        ev = None
+        if slab.world == 1:                     # own faces, own flags: order by event, nothing may spin on this GPU
+            ev = torch.cuda.Event()
+            ev.record(self.side)
+        return _Halos(self._halo(me, gen, 0), self._halo(me, gen, 1), ev, self._flag(me, 0), self._flag(me, 1), self.epoch)
+
+    def after_boundary(self, slab, stream):
+        pass
+
+
+def make_transport(slab, dist, device, kind="auto"):
+    """kind: "peer" (symmetric memory, fails loudly if unavailable), "sendrecv", or "auto" (peer memory if the process
+    group and the devices support it, else send/recv).  Returns (transport, name)."""
+    if kind in ("auto", "peer"):
+        try:
+            return PeerMemoryTransport(slab, dist, device), "peer-memory stores + device-side epoch flags (symmetric memory)"
+        except Exception as e:  # noqa: BLE001 -- any failure of the rendezvous means: no peer mapping on this box
+            if kind == "peer":
+                raise
+            why = f"{type(e).__name__}: {e}"
+            return SendRecvTransport(slab, dist, device), f"ncclSend/ncclRecv (peer memory unavailable: {why[:120]})"
+    return SendRecvTransport(slab, dist, device), "ncclSend/ncclRecv"

@@ -58,37 +58,46 @@ def test_reference_arm_runs_on_rank0_only():
 def _slab_worker(rank, world, port, out):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     sys.path.insert(0, ROOT)
-    from paper_1112_5280_b200.slab import TimeSlab
+    from paper_1112_5280_b200.slab import TimeSlab, SendRecvTransport
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         s = TimeSlab((8, 8, 8, 16), 32, 12, (1, 1, 1, -1), rank, world)   # host-only: no CUDA call is made
-        sb = s.slice_bytes
-        f = torch.empty((s.Tl + 2) * sb, dtype=torch.uint8)
-        for tl in range(s.Tl + 2):                       # byte pattern = 16 * rank + local slice; ghosts 255
-            s.slice_view(f, tl).fill_(255 if tl in (0, s.Tl + 1) else 16 * rank + tl)
-        s.exchange(f, dist)
-        out[rank] = (int(s.slice_view(f, 0)[0]), int(s.slice_view(f, 0)[-1]), int(s.slice_view(f, s.Tl + 1)[0]),
-                     int(s.slice_view(f, s.Tl + 1)[-1]), int(s.slice_view(f, 1)[0]), s.time_indices(), s.local_parity(0))
+        tr = SendRecvTransport(s, dist, "cpu")
+        assert tr.send_up.numel() == s.halo_bytes == 8 * 8 * 8 // 2 * 12 * 4   # projected half spinors: 12 reals per face site
+        tr.send_up.fill_(10 * rank + 1)       # byte patterns: which rank, which face
+        tr.send_down.fill_(10 * rank + 2)
+        tr.from_up.fill_(255)
+        tr.from_down.fill_(255)
+        tr.exchange(s)
+        out[rank] = (int(tr.from_up[0]), int(tr.from_up[-1]), int(tr.from_down[0]), int(tr.from_down[-1]), s.above(), s.below(),
+                     s.time_indices(), s.t_below())
     finally:
         dist.destroy_process_group()
 
 
-def test_time_slab_ghost_exchange_world2():
-    """Ring exchange of the time-slab decomposition (paper_1112_5280_b200/slab.py) over gloo on CPU tensors:
-    ghost 0 receives the left neighbour's last interior slice, ghost Tl + 1 the right neighbour's first."""
-    world, port = 2, _free_port()
+def _check_ring(world):
+    port = _free_port()
     with mp.Manager() as m:
         out = m.dict()
         mp.spawn(_slab_worker, args=(world, port, out), nprocs=world, join=True)
         res = dict(out)
-    Tl = 8
-    for r in range(2):
-        other = 1 - r
-        g0a, g0b, g1a, g1b, own, tidx, lp = res[r]
-        assert g0a == g0b == 16 * other + Tl      # left neighbour (= the other rank on a ring of 2): its slice Tl
-        assert g1a == g1b == 16 * other + 1       # right neighbour: its slice 1
-        assert own == 16 * r + 1                  # interior untouched
-        assert tidx == [(r * Tl - 1 + k) % 16 for k in range(Tl + 2)] and lp == 1
+    Tl = 16 // world
+    for r in range(world):
+        fu0, fu1, fd0, fd1, above, below, tidx, tb = res[r]
+        assert (above, below) == ((r + 1) % world, (r - 1) % world)
+        assert fu0 == fu1 == 10 * above + 2      # from_up: the DOWNWARD face (first slice) of the rank above
+        assert fd0 == fd1 == 10 * below + 1      # from_down: the UPWARD face (last slice) of the rank below
+        assert tidx == list(range(r * Tl, (r + 1) * Tl)) and tb == (r * Tl - 1) % 16
+
+
+def test_time_slab_face_exchange_world2():
+    """Ring exchange of the projected faces (paper_1112_5280_b200/slab.py, SendRecvTransport) over gloo on CPU tensors.  On
+    a ring of two both neighbours are the same rank, so the pairing of the two faces is what this pins."""
+    _check_ring(2)
+
+
+def test_time_slab_face_exchange_world4():
+    _check_ring(4)
 
 
 def test_reference_arm_prints_the_contract_line():
