@@ -61,6 +61,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="lattice_inputs.CONFIGS id of the main workload")
     ap.add_argument("--precision", type=int, default=32, choices=[16, 32, 64], help="precision of the primary line (16: half storage, fp32 arithmetic)")
     ap.add_argument("--recon", type=int, default=12, choices=[8, 12, 18])
+    ap.add_argument("--kernel", default="gather", choices=["gather", "pipe"],
+                    help="lqcd_set_kernel for the primary line and the fp64 / recon legs: gather (one thread per site) or pipe (TMA pipeline)")
     ap.add_argument("--no-extras", action="store_true", help="primary line only (profiling runs)")
     ap.add_argument("--legs", default="all", help="comma list of extra legs: " + ",".join(ALL_LEGS) + " (default all)")
     return ap.parse_args()
@@ -177,7 +179,7 @@ class ClockSampler:
 class Workload:
     """Seeded inputs of one config on the device in native layout, plus pinned host copies."""
 
-    def __init__(self, cfg_id, precision, recon, dev, nbuf=NBUF, keep_host=True, in_parity=None, U=None, link_precision=0):
+    def __init__(self, cfg_id, precision, recon, dev, nbuf=NBUF, keep_host=True, in_parity=None, U=None, link_precision=0, kernel="gather"):
         import numpy as np
         import torch
         import lattice_inputs as li
@@ -188,6 +190,9 @@ class Workload:
         self.precision, self.recon, self.dev, self.nbuf, self.link_precision = precision, recon, dev, nbuf, link_precision
         cd = np.complex128 if precision == 64 else np.complex64  # precision 16 exchanges complex64
         self.ctx = L.Context(self.dims, precision, recon, self.bc, link_precision)
+        if kernel == "pipe" and precision != 16 and not link_precision:
+            self.ctx.set_kernel(L.KERNEL_PIPE)
+        self.kernel = kernel
         self.Vh = self.ctx.Vh
         if U is None:
             U = li.links_for_config(cfg_id, dtype=cd)
@@ -422,10 +427,10 @@ def e2e_leg(torch, w, steps, world):
     }
 
 
-def chain_leg(torch, cfg_id, precision, recon, dev, napply=100, reps=3, U=None):
+def chain_leg(torch, cfg_id, precision, recon, dev, napply=100, reps=3, U=None, kernel="gather"):
     """Config 5 (reading A16): x_{k+1} = M x_k, M = 1 - kappa^2 H_eo H_oe, `napply` times back to back,
     ping-pong buffers, timed as one block; `reps` + 1 blocks, median and min."""
-    w = Workload(cfg_id, precision, recon, dev, nbuf=1, keep_host=False, in_parity=0, U=U)  # even half spinor
+    w = Workload(cfg_id, precision, recon, dev, nbuf=1, keep_host=False, in_parity=0, U=U, kernel=kernel)  # even half spinor
     x, y = w.inp[0], w.out[0]
     ws = torch.empty_like(x)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -624,10 +629,10 @@ def run_b200(args):
     timer = Timer(torch, dist, reduce_device, sampler)
     solo = Timer(torch, None, reduce_device, sampler)   # rank-0-only legs
 
-    w = Workload(args.config, args.precision, args.recon, dev)
+    w = Workload(args.config, args.precision, args.recon, dev, kernel=args.kernel)
     main = kernel_leg(timer, w, args.steps, args.warmup, world, peak, nregions=5, sustained_s=SUSTAINED_S)
     traffic, traffic_src = ncu_traffic(args.precision, args.recon)
-    kname = f"dslash_kernel<fp{args.precision}, recon {args.recon}, EPI_STORE>"
+    kname = f"{'dslash_pipe_kernel' if args.kernel == 'pipe' else 'dslash_kernel'}<fp{args.precision}, recon {args.recon}, EPI_STORE>"
 
     def roofline(r):
         return {"bound": "hbm", "achieved": r["gbs"], "peak": peak, "unit": "GB/s", "frac": r["gbs"] / peak,
@@ -684,7 +689,7 @@ def run_b200(args):
     other = 32 if args.precision == 64 else 64
     w2 = None
     if want("fp64") or want("cgmixed"):
-        w2 = Workload(args.config, other, args.recon, dev, keep_host=False)
+        w2 = Workload(args.config, other, args.recon, dev, keep_host=False, kernel=args.kernel)
     if want("fp64"):
         r2 = kernel_leg(timer, w2, half, args.warmup, world, peak, nregions=5, sustained_s=SUSTAINED_S)
         t2, t2s = ncu_traffic(other, args.recon)
@@ -703,13 +708,13 @@ def run_b200(args):
     torch.cuda.empty_cache()
     if want("recon18"):
         for prec in (32, 64):
-            wv = Workload(args.config, prec, 18, dev, keep_host=False)
+            wv = Workload(args.config, prec, 18, dev, keep_host=False, kernel=args.kernel)
             line[f"recon18_fp{prec}"] = brief(kernel_leg(timer, wv, half, args.warmup, world, peak))
             del wv
             torch.cuda.empty_cache()
     if want("recon8") and getattr(L, "HAS_RECON8", False):
         for prec in (32, 64):
-            wv = Workload(args.config, prec, 8, dev, keep_host=False)
+            wv = Workload(args.config, prec, 8, dev, keep_host=False, kernel=args.kernel)
             line[f"recon8_fp{prec}"] = brief(kernel_leg(timer, wv, half, args.warmup, world, peak))
             del wv
             torch.cuda.empty_cache()
@@ -741,7 +746,7 @@ def run_b200(args):
             t0 = time.perf_counter()
             U5 = li.links_for_config(5, dtype=np.complex64)
             gen_s = time.perf_counter() - t0
-            line["chain"] = [chain_leg(torch, 5, 32, rc, dev, U=U5) for rc in (12, 18)]
+            line["chain"] = [chain_leg(torch, 5, 32, rc, dev, U=U5, kernel=args.kernel) for rc in (12, 18)]
             line["chain_link_generation_s"] = gen_s
             del U5
         if want("cpu"):

@@ -233,6 +233,18 @@ lqcd_status lqcd_dslash_eo_host_batch(const lqcd_ctx* ctx, int n, void* const* o
 lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* ctx, void* out_host, const void* gauge_host,
                                 const void* in_host, int out_parity, void* workspace_dev, void* stream);
 
+/* Which kernel the hot-path entry points of this ctx launch (same arithmetic, same results up to the order of the
+ * floating-point accumulation, which is identical: both add the eight hops in the order x+, x-, y+, y-, z+, z-, t+, t-):
+ *   LQCD_KERNEL_GATHER  one thread per output site, operands gathered into registers (the default)
+ *   LQCD_KERNEL_PIPE    persistent warp-specialised kernel, one CTA per SM: a producer warp stages links and
+ *                       neighbour-spinor tiles in a shared-memory ring with TMA bulk copies (cp.async.bulk + mbarrier),
+ *                       consumer warps compute from shared memory (north_star (3): "shared-memory or TMA staging of
+ *                       neighbour tiles").  Precision 32 / 64 with links of the same precision; otherwise
+ *                       LQCD_EUNSUPPORTED.  The time-slab boundary kernel (lqcd_dslash_eo_slab) is always the gather form. */
+#define LQCD_KERNEL_GATHER 0
+#define LQCD_KERNEL_PIPE 1
+lqcd_status lqcd_set_kernel(lqcd_ctx* ctx, int kernel);
+
 /* Number of kernels this library has launched since load (a claim counter for bench.py). */
 unsigned long long lqcd_launch_count(void);
 

@@ -14,13 +14,14 @@ from . import _build
 
 LQCD_OK, LQCD_EINVAL, LQCD_EALIGN, LQCD_EALIAS, LQCD_EUNSUPPORTED, LQCD_ECUDA = range(6)
 PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, -1
+KERNEL_GATHER, KERNEL_PIPE = 0, 1
 HAS_RECON8 = True
 
 EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
     "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_set_time_slab", "lqcd_dslash_eo_range", "lqcd_pack_gauge_slab", "lqcd_halo_bytes", "lqcd_slab_push_faces", "lqcd_dslash_eo_slab", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_dslash_eo_host_batch", "lqcd_launch_count",
-    "lqcd_gauge_recon8_margin", "lqcd_status_string", "lqcd_last_cuda_error",
+    "lqcd_gauge_recon8_margin", "lqcd_set_kernel", "lqcd_status_string", "lqcd_last_cuda_error",
 ]
 
 
@@ -64,6 +65,7 @@ def _lib():
         lib.lqcd_dslash_eo.argtypes = [vp, vp, vp, vp, ci, vp]
         lib.lqcd_apply_M.argtypes = [vp, vp, vp, vp, cd, ci, vp, vp]
         lib.lqcd_set_time_slab.argtypes = [vp, ci, ci]
+        lib.lqcd_set_kernel.argtypes = [vp, ci]
         lib.lqcd_dslash_eo_range.argtypes = [vp, vp, vp, vp, ci, ci, ci, vp]
         lib.lqcd_halo_bytes.argtypes = [vp]
         lib.lqcd_halo_bytes.restype = sz
@@ -165,6 +167,9 @@ class Context:
     def dslash_eo(self, out, gauge, inp, out_parity, stream=None):
         _chk(_lib().lqcd_dslash_eo(self._h, _ptr(out), _ptr(gauge), _ptr(inp), int(out_parity), _stream(stream)),
              "lqcd_dslash_eo")
+
+    def set_kernel(self, kernel):
+        _chk(_lib().lqcd_set_kernel(self._h, int(kernel)), "lqcd_set_kernel")
 
     def set_time_slab(self, t_cross_fwd, t_cross_bwd):
         _chk(_lib().lqcd_set_time_slab(self._h, int(t_cross_fwd), int(t_cross_bwd)), "lqcd_set_time_slab")

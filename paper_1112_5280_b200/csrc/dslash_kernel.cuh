@@ -96,21 +96,13 @@ __device__ __forceinline__ void project_h(const uint4 w[3], float h[12]) {
     }
 }
 
-// The rest of the arithmetic of one hop on the projected half spinor h and the link u:
-// boundary phase (K3b), colour multiply (K4), reconstruct + accumulate (K5).
-template <typename R, bool CBC, int MU, bool FWD>
-__device__ __forceinline__ void hop_rest(R acc[24], R h[12], R scale, const R u[18], bool cross, const BcPhases<R>& bc) {
-    constexpr int S = FWD ? +1 : -1;
-    using P = Proj<MU>;
-
-    // K3b: psi(x + L mu^) = bc psi(x): forward crossing multiplies by bc_mu, backward by conj(bc_mu).
-    // Real (+-1) phases cost nothing: the sign f rides on the accumulation FMAs of K5.
-    // the neighbour spinor is scale * v (16-bit storage keeps a norm per site; scale = 1 otherwise): the hop is
-    // linear, so the scale rides on f too
-    R f = scale;
+// K3b: psi(x + L mu^) = bc psi(x): forward crossing multiplies by bc_mu = br + i bi, backward by its conjugate (the
+// caller passes -bi).  Real (+-1) phases cost nothing: the sign rides on the accumulation factor f of K5, and so does the
+// site norm of 16-bit storage (the neighbour spinor is scale * v; the hop is linear).  Returns f.
+template <typename R, bool CBC>
+__device__ __forceinline__ R boundary_phase(R h[12], R scale, bool cross, R br, R bi) {
     if (CBC) {
         if (cross) {
-            const R br = bc.re[MU], bi = FWD ? bc.im[MU] : -bc.im[MU];
 #pragma unroll
             for (int k = 0; k < 6; ++k) {
                 const R a = h[2 * k], b = h[2 * k + 1];
@@ -118,12 +110,14 @@ __device__ __forceinline__ void hop_rest(R acc[24], R h[12], R scale, const R u[
                 h[2 * k + 1] = a * bi + b * br;
             }
         }
-    } else {
-        f = cross ? bc.re[MU] * scale : scale;
+        return scale;
     }
+    return cross ? br * scale : scale;
+}
 
-    // K4: chi = U h (forward) or U^+ h (backward), both spin components; explicit FMA chains
-    R chi[12];
+// K4: chi = U h (forward) or U^+ h (backward), both spin components; explicit FMA chains
+template <typename R, bool FWD>
+__device__ __forceinline__ void su3_multiply(const R h[12], const R u[18], R chi[12]) {
 #pragma unroll
     for (int sp = 0; sp < 2; ++sp)
 #pragma unroll
@@ -148,8 +142,12 @@ __device__ __forceinline__ void hop_rest(R acc[24], R h[12], R scale, const R u[
             chi[6 * sp + 2 * a] = cr;
             chi[6 * sp + 2 * a + 1] = ci;
         }
+}
 
-    // K5: out0 += f chi0, out1 += f chi1, out2 += f S c2 chi_k2, out3 += f S c3 chi_k3
+// K5: out0 += f chi0, out1 += f chi1, out2 += f S c2 chi_k2, out3 += f S c3 chi_k3
+template <typename R, int MU, int S>
+__device__ __forceinline__ void reconstruct_accumulate(R acc[24], const R chi[12], R f) {
+    using P = Proj<MU>;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         acc[2 * c] = fma_(f, chi[2 * c], acc[2 * c]);
@@ -159,6 +157,16 @@ __device__ __forceinline__ void hop_rest(R acc[24], R h[12], R scale, const R u[
         cfma<coef_sgn<S>(P::c2)>(acc[12 + 2 * c], acc[12 + 2 * c + 1], f, chi[6 * P::k2 + 2 * c], chi[6 * P::k2 + 2 * c + 1]);
         cfma<coef_sgn<S>(P::c3)>(acc[18 + 2 * c], acc[18 + 2 * c + 1], f, chi[6 * P::k3 + 2 * c], chi[6 * P::k3 + 2 * c + 1]);
     }
+}
+
+// The rest of the arithmetic of one hop on the projected half spinor h and the link u:
+// boundary phase (K3b), colour multiply (K4), reconstruct + accumulate (K5).
+template <typename R, bool CBC, int MU, bool FWD>
+__device__ __forceinline__ void hop_rest(R acc[24], R h[12], R scale, const R u[18], bool cross, const BcPhases<R>& bc) {
+    const R f = boundary_phase<R, CBC>(h, scale, cross, bc.re[MU], FWD ? bc.im[MU] : -bc.im[MU]);
+    R chi[12];
+    su3_multiply<R, FWD>(h, u, chi);
+    reconstruct_accumulate<R, MU, FWD ? +1 : -1>(acc, chi, f);
 }
 
 // 16-bit storage: project with mixed-precision adds on the stored words (1) or convert all 24 components first (0)
@@ -298,6 +306,31 @@ __device__ __forceinline__ void g5_scale(R v[24], R g_re, R g_im) {
     }
 }
 
+// K6 + L6: the epilogue on acc = (H in)(x), then the store (shared by the gather kernel and the pipelined kernel).
+template <typename S, int EPI>
+__device__ __forceinline__ void finish_site(typename Compute<S>::type acc[24], S* __restrict__ out, const S* __restrict__ xin,
+                                            const Epilogue<typename Compute<S>::type>& epi, int ntiles, int cb, bool live) {
+    using R = typename Compute<S>::type;
+    constexpr bool XPAY = EPI == EPI_XPAY || EPI == EPI_G5XPAY;
+    if constexpr (EPI == EPI_G5SCALE) g5_scale<R>(acc, epi.g_re, epi.g_im);
+    if constexpr (XPAY) {
+        R x[24], xs;
+        load_field<S>(xin, ntiles, cb, x, xs);
+        if constexpr (sizeof(S) == 2) {
+#pragma unroll
+            for (int k = 0; k < 24; ++k) x[k] *= xs;
+        }
+        if constexpr (EPI == EPI_G5XPAY) g5_scale<R>(x, epi.g_re, epi.g_im);
+#pragma unroll
+        for (int k = 0; k < 24; ++k) acc[k] = fma_(epi.a, acc[k], x[k]);
+    }
+    if (epi.g5_out) {
+#pragma unroll
+        for (int k = 12; k < 24; ++k) acc[k] = -acc[k];
+    }
+    if (live) store_field<S>(out, ntiles, cb, acc);
+}
+
 // grid.y = 1: one parity `parity0`; grid.y = 2: both, parity = blockIdx.y, and in/out/xin are
 // full fields [even|odd] (in is read at the opposite half).  One thread per output site.
 // S = storage type of all fields (float, double, or __half with fp32 arithmetic), R = arithmetic type.
@@ -328,18 +361,8 @@ dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restr
 
     // K1: all eight neighbours and boundary-crossing flags
     int nb[8];
-    unsigned crossmask = 0;
-    {
-        bool c;
-        nb[0] = neighbour<0, true>(g, cb, s, c);  crossmask |= (unsigned)c << 0;
-        nb[1] = neighbour<0, false>(g, cb, s, c); crossmask |= (unsigned)c << 1;
-        nb[2] = neighbour<1, true>(g, cb, s, c);  crossmask |= (unsigned)c << 2;
-        nb[3] = neighbour<1, false>(g, cb, s, c); crossmask |= (unsigned)c << 3;
-        nb[4] = neighbour<2, true>(g, cb, s, c);  crossmask |= (unsigned)c << 4;
-        nb[5] = neighbour<2, false>(g, cb, s, c); crossmask |= (unsigned)c << 5;
-        nb[6] = neighbour<3, true>(g, cb, s, c);  crossmask |= (unsigned)c << 6;
-        nb[7] = neighbour<3, false>(g, cb, s, c); crossmask |= (unsigned)c << 7;
-    }
+    unsigned crossmask;
+    all_neighbours(g, cb, s, nb, crossmask);
     const auto* site_links = reinterpret_cast<const typename LinkStore<S, RECON>::word*>(gauge) +
                              LinkStore<S, RECON>::word0(g.ntiles, p, cb, 0);
 
@@ -360,23 +383,7 @@ dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restr
     hop_step<S, RECON, CBC, 6>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
     hop_step<S, RECON, CBC, 7>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
 
-    if constexpr (EPI == EPI_G5SCALE) g5_scale<R>(acc, epi.g_re, epi.g_im);
-    if constexpr (XPAY) {
-        R x[24], xs;
-        load_field<S>(xin, g.ntiles, cb, x, xs);
-        if constexpr (sizeof(S) == 2) {
-#pragma unroll
-            for (int k = 0; k < 24; ++k) x[k] *= xs;
-        }
-        if constexpr (EPI == EPI_G5XPAY) g5_scale<R>(x, epi.g_re, epi.g_im);
-#pragma unroll
-        for (int k = 0; k < 24; ++k) acc[k] = fma_(epi.a, acc[k], x[k]);
-    }
-    if (epi.g5_out) {
-#pragma unroll
-        for (int k = 12; k < 24; ++k) acc[k] = -acc[k];
-    }
-    if (live) store_field<S>(out, g.ntiles, cb, acc);
+    finish_site<S, EPI>(acc, out, xin, epi, g.ntiles, cb, live);
 }
 
 }  // namespace lqcd

@@ -17,7 +17,24 @@ struct Geom {
     int sy, sz, st;  // cb strides of y, z, t: Xh, Xh*Y, Xh*Y*Z
     int tcf, tcb;    // t whose forward / backward hop carries the boundary phase: T-1 / 0 on a whole lattice; a
                      // time slab (lqcd_set_time_slab) moves them to where the global boundary cuts it, or -1
+    // division by the run-time extents Xh, Y, Z without a divide: n / d = (n * mul) >> shift for every n < 2^30
+    // (set_fastdiv; checkerboard indices are below 2^30 by lqcd_create)
+    unsigned mul_xh, mul_y, mul_z;
+    int sh_xh, sh_y, sh_z;
 };
+
+// mul = ceil(2^shift / d), shift = 30 + l, l = ceil(log2 d).  With e = mul d - 2^shift in [0, d):
+// n mul / 2^shift = n / d + n e / (d 2^shift), and the excess is below 1 / d for n < 2^30 (n e < 2^30 2^l = 2^shift), so the
+// floor is floor(n / d).  mul <= 2^31 fits in 32 bits.  (Checked against integer division in tests/test_abi.py.)
+inline void set_fastdiv(unsigned d, unsigned& mul, int& shift) {
+    int l = 0;
+    while ((1u << l) < d) ++l;
+    shift = 30 + l;
+    mul = (unsigned)((((unsigned long long)1 << shift) + d - 1) / d);
+}
+__device__ __forceinline__ unsigned fastdiv(unsigned n, unsigned mul, int shift) {
+    return (unsigned)(((unsigned long long)n * mul) >> shift);
+}
 
 struct Site {
     int xh, y, z, t;
@@ -28,13 +45,13 @@ struct Site {
 __device__ __forceinline__ Site decode_site(const Geom& g, int cb, int p) {
     Site s;
     unsigned r = (unsigned)cb;
-    unsigned q = r / (unsigned)g.Xh;
+    unsigned q = fastdiv(r, g.mul_xh, g.sh_xh);
     s.xh = (int)(r - q * (unsigned)g.Xh);
     r = q;
-    q = r / (unsigned)g.Y;
+    q = fastdiv(r, g.mul_y, g.sh_y);
     s.y = (int)(r - q * (unsigned)g.Y);
     r = q;
-    q = r / (unsigned)g.Z;
+    q = fastdiv(r, g.mul_z, g.sh_z);
     s.z = (int)(r - q * (unsigned)g.Z);
     s.t = (int)q;
     s.x_odd = (s.y + s.z + s.t + p) & 1;
@@ -80,6 +97,35 @@ __device__ __forceinline__ int neighbour(const Geom& g, int cb, const Site& s, b
             return (s.t == 0) ? cb + (g.T - 1) * g.st : cb - g.st;
         }
     }
+}
+
+// the neighbour of hop k = 2 mu + (backward ? 1 : 0), k known only at run time (the producer warps of pipe_kernel.cuh)
+__device__ __forceinline__ int neighbour_rt(const Geom& g, int cb, const Site& s, int k) {
+    bool c;
+    switch (k) {
+        case 0: return neighbour<0, true>(g, cb, s, c);
+        case 1: return neighbour<0, false>(g, cb, s, c);
+        case 2: return neighbour<1, true>(g, cb, s, c);
+        case 3: return neighbour<1, false>(g, cb, s, c);
+        case 4: return neighbour<2, true>(g, cb, s, c);
+        case 5: return neighbour<2, false>(g, cb, s, c);
+        case 6: return neighbour<3, true>(g, cb, s, c);
+        default: return neighbour<3, false>(g, cb, s, c);
+    }
+}
+
+// K1 for one site: all eight neighbours (hop k = 2 mu + (backward ? 1 : 0)) and the bit mask of boundary-crossing hops.
+__device__ __forceinline__ void all_neighbours(const Geom& g, int cb, const Site& s, int nb[8], unsigned& crossmask) {
+    bool c;
+    crossmask = 0;
+    nb[0] = neighbour<0, true>(g, cb, s, c);  crossmask |= (unsigned)c << 0;
+    nb[1] = neighbour<0, false>(g, cb, s, c); crossmask |= (unsigned)c << 1;
+    nb[2] = neighbour<1, true>(g, cb, s, c);  crossmask |= (unsigned)c << 2;
+    nb[3] = neighbour<1, false>(g, cb, s, c); crossmask |= (unsigned)c << 3;
+    nb[4] = neighbour<2, true>(g, cb, s, c);  crossmask |= (unsigned)c << 4;
+    nb[5] = neighbour<2, false>(g, cb, s, c); crossmask |= (unsigned)c << 5;
+    nb[6] = neighbour<3, true>(g, cb, s, c);  crossmask |= (unsigned)c << 6;
+    nb[7] = neighbour<3, false>(g, cb, s, c); crossmask |= (unsigned)c << 7;
 }
 
 }  // namespace lqcd

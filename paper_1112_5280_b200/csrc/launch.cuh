@@ -5,11 +5,13 @@
 #include "../../include/lqcd.h"
 
 #include "dslash_kernel.cuh"
+#include "pipe_kernel.cuh"
 
 struct lqcd_ctx {
     lqcd_params p;
     lqcd::Geom g;
     bool complex_bc;
+    int kernel;   // LQCD_KERNEL_GATHER or LQCD_KERNEL_PIPE (lqcd_set_kernel)
 };
 
 namespace lqcd {
@@ -39,9 +41,44 @@ BcPhases<R> make_bc(const lqcd_ctx* c) {
     return b;
 }
 
+// the pipelined kernel exists for fp32 / fp64 fields with links stored in the same precision
+template <typename S, int RECON> constexpr bool pipe_capable = (sizeof(S) == 4 || sizeof(S) == 8) && (RECON == 8 || RECON == 12 || RECON == 18);
+
+// SMs of the current device (persistent grid of the pipelined kernel); 0 on error
+inline int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess) n = v;
+    }
+    return n;
+}
+
+template <typename R, int RECON, int EPI, bool CBC>
+lqcd_status launch_pipe(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                        const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
+    using P = Pipe<R, RECON>;
+    auto kernel = dslash_pipe_kernel<R, RECON, EPI, CBC>;
+    static bool configured = false;
+    if (!configured) {
+        if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, P::SMEM_BYTES) != cudaSuccess) return after_launch();
+        configured = true;
+    }
+    const int nt = ((rg.end + TILE - 1) >> 5) - (rg.begin >> 5), nwork = parity < 0 ? 2 * nt : nt;
+    const int nsm = sm_count();
+    if (nsm <= 0) return LQCD_ECUDA;
+    const Epilogue<R> epi{(R)e.a, (R)e.g_re, (R)e.g_im, e.g5_out};
+    kernel<<<nwork < nsm ? nwork : nsm, P::THREADS, P::SMEM_BYTES, st>>>((R*)out, (const R*)gauge, (const R*)in, (const R*)xin, epi, c->g,
+                                                                        parity < 0 ? 0 : parity, parity < 0 ? 1 : 0, make_bc<R>(c), rg.begin, rg.end);
+    return after_launch();
+}
+
 template <typename S, int RECON, int EPI, bool CBC>
 lqcd_status launch_one(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
                        const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
+    if constexpr (pipe_capable<S, RECON>) {
+        if (c->kernel == LQCD_KERNEL_PIPE) return launch_pipe<S, RECON, EPI, CBC>(c, out, gauge, in, xin, e, parity, st, rg);
+    }
     constexpr int BLOCK = DSLASH_BLOCK;
     const dim3 grid((rg.end - rg.begin + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
     using A = typename Compute<S>::type;  // S is the storage type, A the arithmetic type

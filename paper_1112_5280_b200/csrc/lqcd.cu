@@ -126,7 +126,11 @@ lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p) {
     g.ntiles = (g.Vh + TILE - 1) / TILE;
     g.sy = g.Xh; g.sz = g.Xh * g.Y; g.st = g.Xh * g.Y * g.Z;
     g.tcf = g.T - 1; g.tcb = 0;
+    set_fastdiv((unsigned)g.Xh, g.mul_xh, g.sh_xh);
+    set_fastdiv((unsigned)g.Y, g.mul_y, g.sh_y);
+    set_fastdiv((unsigned)g.Z, g.mul_z, g.sh_z);
     c->complex_bc = cbc;
+    c->kernel = LQCD_KERNEL_GATHER;
     *ctx = c;
     return LQCD_OK;
 }
@@ -228,6 +232,13 @@ lqcd_status lqcd_pack_spinor(const lqcd_ctx* c, void* native, const void* canon,
 
 lqcd_status lqcd_unpack_spinor(const lqcd_ctx* c, void* canon, const void* native, int parity, void* stream) {
     return pack_unpack(c, canon, native, parity, stream, true);
+}
+
+lqcd_status lqcd_set_kernel(lqcd_ctx* c, int kernel) {
+    if (!c || (kernel != LQCD_KERNEL_GATHER && kernel != LQCD_KERNEL_PIPE)) return LQCD_EINVAL;
+    if (kernel == LQCD_KERNEL_PIPE && (c->p.precision == 16 || c->p.link_precision == 16)) return LQCD_EUNSUPPORTED;
+    c->kernel = kernel;
+    return LQCD_OK;
 }
 
 lqcd_status lqcd_dslash_full(const lqcd_ctx* c, void* out, const void* gauge, const void* in, void* stream) {

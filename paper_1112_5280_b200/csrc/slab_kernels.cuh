@@ -133,18 +133,8 @@ dslash_slab_kernel(R* __restrict__ out, const R* __restrict__ gauge, const R* __
     if (cb >= cb_end) return;
     const Site s = decode_site(g, cb, p);
     int nb[8];
-    unsigned crossmask = 0;
-    {
-        bool c;
-        nb[0] = neighbour<0, true>(g, cb, s, c);  crossmask |= (unsigned)c << 0;
-        nb[1] = neighbour<0, false>(g, cb, s, c); crossmask |= (unsigned)c << 1;
-        nb[2] = neighbour<1, true>(g, cb, s, c);  crossmask |= (unsigned)c << 2;
-        nb[3] = neighbour<1, false>(g, cb, s, c); crossmask |= (unsigned)c << 3;
-        nb[4] = neighbour<2, true>(g, cb, s, c);  crossmask |= (unsigned)c << 4;
-        nb[5] = neighbour<2, false>(g, cb, s, c); crossmask |= (unsigned)c << 5;
-        nb[6] = neighbour<3, true>(g, cb, s, c);  crossmask |= (unsigned)c << 6;
-        nb[7] = neighbour<3, false>(g, cb, s, c); crossmask |= (unsigned)c << 7;
-    }
+    unsigned crossmask;
+    all_neighbours(g, cb, s, nb, crossmask);
     const auto* site_links = reinterpret_cast<const typename LinkStore<R, RECON>::word*>(gauge) +
                              LinkStore<R, RECON>::word0(g.ntiles, p, cb, 0);
     R acc[24];

@@ -5,6 +5,8 @@ and the hot-path entry points of paper_1112_5280_b200.
 """
 from __future__ import annotations
 
+import os
+
 import numpy as np
 import torch
 
@@ -32,8 +34,14 @@ def scatter_half(half: np.ndarray, dims, parity: int) -> np.ndarray:
 class Gpu:
     """One context plus the packed gauge field on cuda:0."""
 
-    def __init__(self, dims, precision, recon, bc, U: np.ndarray, link_precision=0):
+    def __init__(self, dims, precision, recon, bc, U: np.ndarray, link_precision=0, kernel=None):
         self.ctx = L.Context(dims, precision, recon, bc, link_precision)
+        # kernel: "gather" / "pipe" (lqcd_set_kernel); None: $LQCD_TEST_KERNEL where the ctx supports it (lets the whole
+        # suite be re-run on the pipelined kernel), else the library default
+        if kernel is None and precision != 16 and not link_precision:
+            kernel = os.environ.get("LQCD_TEST_KERNEL")
+        if kernel is not None:
+            self.ctx.set_kernel({"gather": L.KERNEL_GATHER, "pipe": L.KERNEL_PIPE}[kernel])
         self.dims, self.precision = tuple(dims), precision
         self.cd = cdtype(precision)
         self.dev = torch.device("cuda:0")
