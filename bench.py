@@ -61,7 +61,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="lattice_inputs.CONFIGS id of the main workload")
     ap.add_argument("--precision", type=int, default=32, choices=[16, 32, 64], help="precision of the primary line (16: half storage, fp32 arithmetic)")
     ap.add_argument("--recon", type=int, default=12, choices=[8, 12, 18])
-    ap.add_argument("--kernel", default="gather", choices=["gather", "pipe"],
+    ap.add_argument("--kernel", default="gather", choices=["gather", "pipe", "blocked"],
                     help="lqcd_set_kernel for the primary line and the fp64 / recon legs: gather (one thread per site) or pipe (TMA pipeline)")
     ap.add_argument("--no-extras", action="store_true", help="primary line only (profiling runs)")
     ap.add_argument("--legs", default="all", help="comma list of extra legs: " + ",".join(ALL_LEGS) + " (default all)")
@@ -192,6 +192,8 @@ class Workload:
         self.ctx = L.Context(self.dims, precision, recon, self.bc, link_precision)
         if kernel == "pipe" and precision != 16 and not link_precision:
             self.ctx.set_kernel(L.KERNEL_PIPE)
+        if kernel == "blocked":
+            self.ctx.set_kernel(L.KERNEL_BLOCKED)
         self.kernel = kernel
         self.Vh = self.ctx.Vh
         if U is None:

@@ -243,6 +243,7 @@ lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* ctx, void* out_host, const void*
  *                       LQCD_EUNSUPPORTED.  The time-slab boundary kernel (lqcd_dslash_eo_slab) is always the gather form. */
 #define LQCD_KERNEL_GATHER 0
 #define LQCD_KERNEL_PIPE 1
+#define LQCD_KERNEL_BLOCKED 2 /* the gather kernel with the blocked thread -> site map (4-D boxes of warp tiles per block) */
 lqcd_status lqcd_set_kernel(lqcd_ctx* ctx, int kernel);
 
 /* Number of kernels this library has launched since load (a claim counter for bench.py). */

@@ -331,6 +331,14 @@ __device__ __forceinline__ void finish_site(typename Compute<S>::type acc[24], S
     if (live) store_field<S>(out, ntiles, cb, acc);
 }
 
+// Thread -> site maps.  Linear: thread t of block b works on checkerboard site cb_begin + b BLOCK + t (a block is a run of
+// consecutive sites: 4 x-rows at 32^3 x 64).  Blocked (whole-lattice launches on lattices whose z planes are multiples of
+// 32 sites): the warp tiles form a 3-D grid (ny tiles per z plane) x Z x T, and a block of by bz bt warps takes a compact
+// by x bz x bt box of it -- a 4-D sub-volume of the lattice -- so that the neighbour spinors its warps gather are to a
+// large part the same tiles and are served by the SM's L1 instead of crossing the L2 -> SM crossbar again (the kernel is
+// bound by that crossbar, not by HBM: DESIGN.md section 6).  by = 0: linear.
+struct BlockMap { int by, bz, bt, ny, gy, gz; };   // box shape in tiles; tiles per z plane; blocks along y, z
+
 // grid.y = 1: one parity `parity0`; grid.y = 2: both, parity = blockIdx.y, and in/out/xin are
 // full fields [even|odd] (in is read at the opposite half).  One thread per output site.
 // S = storage type of all fields (float, double, or __half with fp32 arithmetic), R = arithmetic type.
@@ -338,7 +346,7 @@ template <typename S, int RECON, int EPI, bool CBC, int BLOCK>
 __global__ void __launch_bounds__(BLOCK, MinBlocks<S, RECON>::value * 64 / BLOCK)
 dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restrict__ in, const S* __restrict__ xin,
               Epilogue<typename Compute<S>::type> epi, Geom g, int parity0, BcPhases<typename Compute<S>::type> bc,
-              int cb_begin, int cb_end) {
+              int cb_begin, int cb_end, BlockMap map) {
     using R = typename Compute<S>::type;
     constexpr bool XPAY = EPI == EPI_XPAY || EPI == EPI_G5XPAY;
     int p = parity0;
@@ -350,6 +358,14 @@ dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restr
         if (XPAY) xin += (size_t)p * half;
     }
     int cb = cb_begin + blockIdx.x * BLOCK + threadIdx.x;  // [cb_begin, cb_end): all sites, or a range of time slices
+    if (map.by) {
+        const int w = threadIdx.x >> 5, b = blockIdx.x;
+        const int wy = w % map.by, wz = (w / map.by) % map.bz, wt = w / (map.by * map.bz);
+        const int gy = b % map.gy, gz = (b / map.gy) % map.gz, gt = b / (map.gy * map.gz);
+        const int ty = gy * map.by + wy, tz = gz * map.bz + wz, tt = gt * map.bt + wt;
+        if (ty >= map.ny || tz >= g.Z || tt >= g.T) return;   // boxes that stick out of the lattice (warp-uniform)
+        cb = (ty + map.ny * (tz + g.Z * tt)) * TILE + (int)(threadIdx.x & 31u);
+    }
     constexpr bool SHFLX = LQCD_SHFL_X && sizeof(S) != 2 && !half_links<S, RECON>;
     bool live = true;
     if (cb >= cb_end) {

@@ -2,6 +2,9 @@
 // instantiation units inst_*.cu (one per storage type x link format, so that the library builds in parallel:
 // each unit instantiates dslash_kernel for its 4 epilogues x 2 boundary-phase kinds).
 #pragma once
+#include <cstdio>
+#include <cstdlib>
+
 #include "../../include/lqcd.h"
 
 #include "dslash_kernel.cuh"
@@ -73,18 +76,44 @@ lqcd_status launch_pipe(const lqcd_ctx* c, void* out, const void* gauge, const v
     return after_launch();
 }
 
+// Box of nwarps warp tiles for the blocked map: 2 tiles along y and 2 along t where the block has the warps for it, the
+// rest along z ($LQCD_BOX = "by,bz,bt" overrides, for sweeps).
+inline BlockMap box_shape(int nwarps, const Geom& g) {
+    BlockMap m;
+    m.ny = g.sz / TILE;
+    m.by = nwarps >= 4 && m.ny >= 2 ? 2 : 1;
+    m.bt = nwarps >= 8 ? 2 : 1;
+    m.bz = nwarps / (m.by * m.bt);
+    if (const char* e = std::getenv("LQCD_BOX")) {
+        int a, b, c2;
+        if (std::sscanf(e, "%d,%d,%d", &a, &b, &c2) == 3 && a > 0 && b > 0 && c2 > 0 && a * b * c2 <= nwarps) { m.by = a; m.bz = b; m.bt = c2; }
+    }
+    m.gy = (m.ny + m.by - 1) / m.by;
+    m.gz = (g.Z + m.bz - 1) / m.bz;
+    return m;
+}
+
 template <typename S, int RECON, int EPI, bool CBC>
 lqcd_status launch_one(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
                        const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
     if constexpr (pipe_capable<S, RECON>) {
         if (c->kernel == LQCD_KERNEL_PIPE) return launch_pipe<S, RECON, EPI, CBC>(c, out, gauge, in, xin, e, parity, st, rg);
     }
-    constexpr int BLOCK = DSLASH_BLOCK;
-    const dim3 grid((rg.end - rg.begin + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
     using A = typename Compute<S>::type;  // S is the storage type, A the arithmetic type
     const Epilogue<A> epi{(A)e.a, (A)e.g_re, (A)e.g_im, e.g5_out};
+    // blocked map: all warps the register budget allows per SM in ONE block, on a compact box of warp tiles
+    constexpr int NWARPS = MinBlocks<S, RECON>::value * 2;
+    if (c->kernel == LQCD_KERNEL_BLOCKED && rg.begin == 0 && rg.end == c->g.Vh && c->g.sz % TILE == 0) {
+        BlockMap m = box_shape(NWARPS, c->g);
+        const dim3 grid(m.gy * m.gz * ((c->g.T + m.bt - 1) / m.bt), parity < 0 ? 2 : 1);
+        dslash_kernel<S, RECON, EPI, CBC, 32 * NWARPS><<<grid, 32 * NWARPS, 0, st>>>(
+            (S*)out, (const S*)gauge, (const S*)in, (const S*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<A>(c), rg.begin, rg.end, m);
+        return after_launch();
+    }
+    constexpr int BLOCK = DSLASH_BLOCK;
+    const dim3 grid((rg.end - rg.begin + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
     dslash_kernel<S, RECON, EPI, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
-        (S*)out, (const S*)gauge, (const S*)in, (const S*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<A>(c), rg.begin, rg.end);
+        (S*)out, (const S*)gauge, (const S*)in, (const S*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<A>(c), rg.begin, rg.end, BlockMap{0, 0, 0, 0, 0, 0});
     return after_launch();
 }
 

@@ -235,7 +235,7 @@ lqcd_status lqcd_unpack_spinor(const lqcd_ctx* c, void* canon, const void* nativ
 }
 
 lqcd_status lqcd_set_kernel(lqcd_ctx* c, int kernel) {
-    if (!c || (kernel != LQCD_KERNEL_GATHER && kernel != LQCD_KERNEL_PIPE)) return LQCD_EINVAL;
+    if (!c || (kernel != LQCD_KERNEL_GATHER && kernel != LQCD_KERNEL_PIPE && kernel != LQCD_KERNEL_BLOCKED)) return LQCD_EINVAL;
     if (kernel == LQCD_KERNEL_PIPE && (c->p.precision == 16 || c->p.link_precision == 16)) return LQCD_EUNSUPPORTED;
     c->kernel = kernel;
     return LQCD_OK;
