@@ -706,6 +706,10 @@ def run_b200(args):
             w32h = Workload(args.config, 32, 12, dev, keep_host=False, nbuf=1, link_precision=16)
             line["cg_mixed_half_links"] = cg_mixed_leg(torch, w64, w32h, tol=1e-10)
             del w32h
+            # 16-bit solver (next row f4): inner CG on 16-bit operator fields, fp32 iterate and residual
+            w16 = Workload(args.config, 16, 12, dev, keep_host=False, nbuf=1)
+            line["cg_mixed_16bit"] = cg_mixed_leg(torch, w64, w16, tol=1e-10, inner_tol=1e-3)
+            del w16
     del w2
     torch.cuda.empty_cache()
     if want("recon18"):

@@ -77,7 +77,7 @@ typedef struct {
     int dims[4];      /* X,Y,Z,T (mu = 0..3); each even and >= 4 (reading A17) */
     int precision;    /* 64 or 32: storage and arithmetic type of all fields; 16: fields stored as IEEE half
                          (spinors normalised per site, with an fp32 norm), fp32 arithmetic, recon 12 only;
-                         canonical buffers are complex64; the CG entry points return LQCD_EUNSUPPORTED */
+                         canonical buffers are complex64; the CG iterates in fp32 on 16-bit operator fields */
     int recon;        /* 18, 12 or 8: stored reals per link; 12 = two rows, third rebuilt in
                          registers as conj(row0 x row1) ("RECONSTRUCT TWELVE"); 8 = the minimal
                          parametrisation of ref. [3]: U01, U02, U10 and the phases of U00, U20,
@@ -197,7 +197,12 @@ lqcd_status lqcd_apply_Q_tm(const lqcd_ctx* ctx, void* out_dev, const void* gaug
  * iterations (every iteration once |r|^2 is within 1000x of the target), and iterations enqueued after convergence
  * leave x untouched.  Reductions are deterministic.
  * The call synchronises `stream` before returning: *iters_out = iterations performed, *relres_out = |r| / |b|
- * of the recursive residual (host pointers, either may be NULL).  Arithmetic in the ctx precision. */
+ * of the recursive residual (host pointers, either may be NULL).  Arithmetic in the ctx precision.
+ * Precision 16 (16-bit solver, PAPER.md:89 ref. [3]): x_dev and b_dev are 16-bit native half spinors; b is widened to fp32,
+ * the iterate x and the residual r are kept in fp32 (their recurrences carry the accuracy), the search direction p, Q p
+ * and A p live in the 16-bit format the operator reads and writes; x is rounded to the 16-bit format at the end.  The
+ * recursive residual then drifts from the true one at the 1e-3 level: use it as the inner solver of
+ * lqcd_cg_solve_tm_mixed, or with tol >= 1e-3. */
 size_t lqcd_cg_workspace_bytes(const lqcd_ctx* ctx);
 lqcd_status lqcd_cg_solve_tm(const lqcd_ctx* ctx, void* x_dev, const void* gauge_dev, const void* b_dev, double kappa,
                              double mu, double tol, int maxiter, void* workspace_dev, int* iters_out,
@@ -208,8 +213,8 @@ lqcd_status lqcd_cg_solve_tm(const lqcd_ctx* ctx, void* x_dev, const void* gauge
  *   x = 0, r = b;  repeat { fp32 CG on A e = (float) r to relative tolerance inner_tol;  x += e;  r = b - A x in fp64 }
  *   until |r| <= tol |b| (r is the TRUE fp64 residual), the total inner iteration count reaches maxiter, or a
  *   correction brings no progress.
- * ctx64 / ctx32: contexts of precision 64 / 32 with the same extents and boundary phases (each with its own
- * recon); gauge64_dev / gauge32_dev: the link field packed for each; x_dev, b_dev: fp64 native even half spinors.
+ * ctx64 / ctx32: contexts of precision 64 and of precision 32 or 16 with the same extents and boundary phases (each with
+ * its own recon; precision 16: the inner iteration keeps x, r in fp32 and p, Q p, A p in 16-bit storage); gauge64_dev / gauge32_dev: the link field packed for each; x_dev, b_dev: fp64 native even half spinors.
  * workspace_dev: lqcd_cg_mixed_workspace_bytes bytes, 256-byte aligned.  Synchronises `stream`.
  * *iters_out = total inner iterations, *outer_out = corrections applied, *relres_out = |b - A x| / |b|. */
 size_t lqcd_cg_mixed_workspace_bytes(const lqcd_ctx* ctx64, const lqcd_ctx* ctx32);

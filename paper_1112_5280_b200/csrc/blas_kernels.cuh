@@ -40,6 +40,23 @@ __device__ __forceinline__ double block_sum(double v) {
     return v;
 }
 
+// A site of a native half spinor as numbers of the arithmetic type A = Compute<S>::type, for any storage type S (float,
+// double, or __half = 16-bit storage: 24 normalised halfs and an fp32 site norm; the store re-normalises and rounds).
+// RW: the calling kernel also writes the field -- coherent loads instead of the read-only path.
+template <typename S, bool RW>
+__device__ __forceinline__ void load_vec(const S* base, int ntiles, int cb, typename Compute<S>::type v[24]) {
+    if constexpr (sizeof(S) == 2) {
+        float n;
+        if constexpr (RW) load_spinor_h_rw(base, ntiles, cb, v, n); else load_spinor_h(base, ntiles, cb, v, n);
+#pragma unroll
+        for (int k = 0; k < 24; ++k) v[k] *= n;
+    } else if constexpr (RW) {
+        load_spinor_rw<S>(base, cb, v);
+    } else {
+        load_spinor<S>(base, cb, v);
+    }
+}
+
 template <typename R>
 __device__ __forceinline__ double site_norm2(const R v[24]) {
     double s = 0.0;
@@ -49,14 +66,15 @@ __device__ __forceinline__ double site_norm2(const R v[24]) {
 }
 
 // partial[blockIdx.x] = sum over the block's sites of |v(x)|^2
-template <typename R>
-__global__ void __launch_bounds__(BLAS_BLOCK) norm2_kernel(const R* __restrict__ v, Geom g, double* __restrict__ partial) {
+template <typename S>
+__global__ void __launch_bounds__(BLAS_BLOCK) norm2_kernel(const S* __restrict__ v, Geom g, double* __restrict__ partial) {
+    using A = typename Compute<S>::type;
     const int cb = blockIdx.x * BLAS_BLOCK + threadIdx.x;
     double s = 0.0;
     if (cb < g.Vh) {
-        R a[24];
-        load_spinor<R>(v, cb, a);
-        s = site_norm2<R>(a);
+        A a[24];
+        load_vec<S, false>(v, g.ntiles, cb, a);
+        s = site_norm2<A>(a);
     }
     s = block_sum(s);
     if (threadIdx.x == 0) partial[blockIdx.x] = s;
@@ -84,64 +102,70 @@ __global__ void __launch_bounds__(BLAS_BLOCK) cg_scalar_kernel(const double* __r
 }
 
 // x += alpha p;  r -= alpha s;  partial = block sums of |r|^2       (skipped once done)
-template <typename R>
-__global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(R* x, R* r, const R* __restrict__ p,
-                                                                   const R* __restrict__ s, Geom g, const CgScalars* __restrict__ sc,
+// X: storage of the iterate and the residual; P: storage of the search direction and of A p (the 16-bit solver keeps
+// x and r in fp32 -- their recurrences carry the accuracy -- and p, A p in the operator's 16-bit format)
+template <typename X, typename P>
+__global__ void __launch_bounds__(BLAS_BLOCK) cg_update_xr_kernel(X* x, X* r, const P* __restrict__ p,
+                                                                   const P* __restrict__ s, Geom g, const CgScalars* __restrict__ sc,
                                                                    double* __restrict__ partial) {
+    using A = typename Compute<X>::type;
     const int cb = blockIdx.x * BLAS_BLOCK + threadIdx.x;
     const bool done = sc->done != 0;
-    const R alpha = (R)sc->alpha;
+    const A alpha = (A)sc->alpha;
     double n2 = 0.0;
     if (cb < g.Vh) {
-        R rv[24];
-        load_spinor_rw<R>(r, cb, rv);   // r and x are updated in place: coherent loads, not .nc
+        A rv[24];
+        load_vec<X, true>(r, g.ntiles, cb, rv);   // r and x are updated in place: coherent loads, not .nc
         if (!done) {
-            R xv[24], pv[24], sv[24];
-            load_spinor_rw<R>(x, cb, xv);
-            load_spinor<R>(p, cb, pv);
-            load_spinor<R>(s, cb, sv);
+            A xv[24];
+            typename Compute<P>::type pv[24], sv[24];
+            load_vec<X, true>(x, g.ntiles, cb, xv);
+            load_vec<P, false>(p, g.ntiles, cb, pv);
+            load_vec<P, false>(s, g.ntiles, cb, sv);
 #pragma unroll
             for (int k = 0; k < 24; ++k) {
-                xv[k] = fmar(alpha, pv[k], xv[k]);
-                rv[k] = fmar(-alpha, sv[k], rv[k]);
+                xv[k] = fmar(alpha, (A)pv[k], xv[k]);
+                rv[k] = fmar(-alpha, (A)sv[k], rv[k]);
             }
-            store_spinor<R>(x, cb, xv);
-            store_spinor<R>(r, cb, rv);
+            store_field<X>(x, g.ntiles, cb, xv);
+            store_field<X>(r, g.ntiles, cb, rv);
         }
-        n2 = site_norm2<R>(rv);
+        n2 = site_norm2<A>(rv);
     }
     n2 = block_sum(n2);
     if (threadIdx.x == 0) partial[blockIdx.x] = n2;
 }
 
 // p = r + beta p       (skipped once done)
-template <typename R>
-__global__ void __launch_bounds__(BLAS_BLOCK) cg_update_p_kernel(R* p, const R* __restrict__ r, Geom g,
+template <typename X, typename P>
+__global__ void __launch_bounds__(BLAS_BLOCK) cg_update_p_kernel(P* p, const X* __restrict__ r, Geom g,
                                                                   const CgScalars* __restrict__ sc) {
+    using A = typename Compute<P>::type;
     const int cb = blockIdx.x * BLAS_BLOCK + threadIdx.x;
     if (cb >= g.Vh || sc->done) return;
-    const R beta = (R)sc->beta;
-    R pv[24], rv[24];
-    load_spinor_rw<R>(p, cb, pv);   // p is updated in place
-    load_spinor<R>(r, cb, rv);
+    const A beta = (A)sc->beta;
+    A pv[24];
+    typename Compute<X>::type rv[24];
+    load_vec<P, true>(p, g.ntiles, cb, pv);   // p is updated in place
+    load_vec<X, false>(r, g.ntiles, cb, rv);
 #pragma unroll
-    for (int k = 0; k < 24; ++k) pv[k] = fmar(beta, pv[k], rv[k]);
-    store_spinor<R>(p, cb, pv);
+    for (int k = 0; k < 24; ++k) pv[k] = fmar(beta, pv[k], (A)rv[k]);
+    store_field<P>(p, g.ntiles, cb, pv);
 }
 
 // ---- mixed-precision defect correction (fp64 outer, fp32 inner CG) -------------------------------------
 
-// dst = (Rd) src, site by site (the two precisions have different words per site in the native layout)
-template <typename Rd, typename Rs>
-__global__ void __launch_bounds__(BLAS_BLOCK) convert_kernel(Rd* __restrict__ dst, const Rs* __restrict__ src, Geom g) {
+// dst = src converted to dst's storage type, site by site (the formats have different words per site in the native layout)
+template <typename Sd, typename Ss>
+__global__ void __launch_bounds__(BLAS_BLOCK) convert_kernel(Sd* __restrict__ dst, const Ss* __restrict__ src, Geom g) {
     const int cb = blockIdx.x * BLAS_BLOCK + threadIdx.x;
     if (cb >= g.Vh) return;
-    Rs a[24];
-    Rd b[24];
-    load_spinor<Rs>(src, cb, a);
+    typename Compute<Ss>::type a[24];
+    typename Compute<Sd>::type b[24];
+    load_vec<Ss, false>(src, g.ntiles, cb, a);
 #pragma unroll
-    for (int k = 0; k < 24; ++k) b[k] = (Rd)a[k];
-    store_spinor<Rd>(dst, cb, b);
+    for (int k = 0; k < 24; ++k) b[k] = (typename Compute<Sd>::type)a[k];
+    store_field<Sd>(dst, g.ntiles, cb, b);
 }
 
 // x += (double) e

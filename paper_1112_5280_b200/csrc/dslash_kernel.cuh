@@ -169,9 +169,125 @@ __device__ __forceinline__ void hop_rest(R acc[24], R h[12], R scale, const R u[
     reconstruct_accumulate<R, MU, FWD ? +1 : -1>(acc, chi, f);
 }
 
-// 16-bit storage: project with mixed-precision adds on the stored words (1) or convert all 24 components first (0)
+// 16-bit storage, arithmetic on the stored operands (LQCD_F16_MIXED = 2).  Blackwell multiplies two f16 operands into an
+// f32 accumulator (fma.rn.f32.f16 -> FHFMA; either half of a 32-bit register, with negation, is an operand): the
+// product of two 11-bit significands is exact in f32, so the SU(3) multiply needs no conversion of the links or of the
+// half spinor at all -- provided the half spinor is an f16 quantity.  So: K3 projects in packed half arithmetic
+// (h = v_a + c v_b rounded once to f16; 6 instructions per hop instead of 24 conversions + 12 adds), K2 rebuilds the
+// third link row in f32 from exact f16 products and rounds it to f16 like the two stored rows, K4 runs on FHFMA with
+// f32 accumulation, K5 and the epilogue stay f32.  Two roundings to an 11-bit significand are added per hop (the
+// projected half spinor and the rebuilt row); DESIGN.md "16-bit storage" derives what they cost: ~1.5e-4 in rel-L2.
+__device__ __forceinline__ float fhfma(unsigned short a, unsigned short b, float c) {
+    float r; asm("fma.rn.f32.f16 %0, %1, %2, %3;" : "=f"(r) : "h"(a), "h"(b), "f"(c)); return r;
+}
+__device__ __forceinline__ float fhfnma(unsigned short a, unsigned short b, float c) {   // c - a b
+    float r; asm("{ .reg .f16 t; neg.f16 t, %1; fma.rn.f32.f16 %0, t, %2, %3; }" : "=f"(r) : "h"(a), "h"(b), "f"(c)); return r;
+}
+__device__ __forceinline__ unsigned short lo16(unsigned x) { return (unsigned short)(x & 0xffffu); }
+__device__ __forceinline__ unsigned short hi16(unsigned x) { return (unsigned short)(x >> 16); }
+
+// a + C b for a unit coefficient C on packed f16 complex numbers (re low, im high), rounded to f16
+template <int C>
+__device__ __forceinline__ unsigned cmix_hh(unsigned a, unsigned b) {
+    const __half2 A = *reinterpret_cast<const __half2*>(&a), B = *reinterpret_cast<const __half2*>(&b);
+    __half2 r;
+    if (C == C_P1) r = __hadd2(A, B);
+    else if (C == C_M1) r = __hsub2(A, B);
+    else if (C == C_PI) r = __hfma2(__lowhigh2highlow(B), __floats2half2_rn(-1.f, 1.f), A);   // (ar - bi, ai + br)
+    else r = __hfma2(__lowhigh2highlow(B), __floats2half2_rn(1.f, -1.f), A);                 // (ar + bi, ai - br)
+    return *reinterpret_cast<const unsigned*>(&r);
+}
+
+// K3 on the stored words: hh[3 sp + c] = packed f16 complex, spin component sp of the projected half spinor
+template <int MU, int S>
+__device__ __forceinline__ void project_hh(const uint4 w[3], unsigned hh[6]) {
+    using P = Proj<MU>;
+    const unsigned* k = reinterpret_cast<const unsigned*>(w);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        hh[c] = cmix_hh<coef_sgn<S>(P::ca)>(k[c], k[3 * P::ja + c]);
+        hh[3 + c] = cmix_hh<coef_sgn<S>(P::cb)>(k[3 + c], k[3 * P::jb + c]);
+    }
+}
+
+// L1 + K2: the two stored rows as 6 packed f16 complex numbers u[3 row + col], the third row rebuilt as
+// conj(row0 x row1) in f32 (exact products) and rounded to f16: u[6 + col]
+__device__ __forceinline__ void load_link_hh(const uint2* __restrict__ site_links, int k, unsigned u[9]) {
+#pragma unroll
+    for (int w = 0; w < 3; ++w) {
+        const uint2 x = __ldcs(site_links + (k * 3 + w) * TILE);
+        u[2 * w] = x.x;
+        u[2 * w + 1] = x.y;
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        const unsigned A = u[a], B = u[b], C = u[3 + b], D = u[3 + a];
+        float re = fhfma(lo16(A), lo16(C), 0.f);
+        re = fhfnma(hi16(A), hi16(C), re);
+        re = fhfnma(lo16(B), lo16(D), re);
+        re = fhfma(hi16(B), hi16(D), re);
+        float im = fhfma(lo16(A), hi16(C), 0.f);
+        im = fhfma(hi16(A), lo16(C), im);
+        im = fhfnma(lo16(B), hi16(D), im);
+        im = fhfnma(hi16(B), lo16(D), im);
+        const __half2 r = __floats2half2_rn(re, -im);
+        u[6 + c] = *reinterpret_cast<const unsigned*>(&r);
+    }
+}
+
+// K4 on f16 operands, f32 accumulation: chi = U h (forward) or U^+ h (backward)
+template <bool FWD>
+__device__ __forceinline__ void su3_multiply_hh(const unsigned hh[6], const unsigned u[9], float chi[12]) {
+#pragma unroll
+    for (int sp = 0; sp < 2; ++sp)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            float cr = 0.f, ci = 0.f;
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const unsigned h = hh[3 * sp + b], U = FWD ? u[3 * a + b] : u[3 * b + a];
+                if (FWD) {   // (ur + i ui)(hr + i hi)
+                    cr = fhfma(lo16(U), lo16(h), cr);
+                    cr = fhfnma(hi16(U), hi16(h), cr);
+                    ci = fhfma(lo16(U), hi16(h), ci);
+                    ci = fhfma(hi16(U), lo16(h), ci);
+                } else {     // (ur - i ui)(hr + i hi)
+                    cr = fhfma(lo16(U), lo16(h), cr);
+                    cr = fhfma(hi16(U), hi16(h), cr);
+                    ci = fhfma(lo16(U), hi16(h), ci);
+                    ci = fhfnma(hi16(U), lo16(h), ci);
+                }
+            }
+            chi[6 * sp + 2 * a] = cr;
+            chi[6 * sp + 2 * a + 1] = ci;
+        }
+}
+
+// one hop of the 16-bit kernel on stored operands
+template <bool CBC, int K>
+__device__ __forceinline__ void hop_step_hh(float acc[24], const uint2* __restrict__ site_links, const __half* __restrict__ in, int ntiles,
+                                            const int nb[8], unsigned crossmask, const BcPhases<float>& bc) {
+    constexpr int MU = K / 2;
+    constexpr bool FWD = (K & 1) == 0;
+    uint4 w[3];
+    float scale;
+    load_words_h(in, ntiles, nb[K], w, scale);
+    unsigned hh[6], u[9];
+    project_hh<MU, FWD ? +1 : -1>(w, hh);
+    load_link_hh(site_links, K, u);
+    float chi[12];
+    su3_multiply_hh<FWD>(hh, u, chi);
+    // K3b on chi instead of h (the multiply is linear): psi(x + L mu^) = bc psi(x)
+    const bool cross = (crossmask >> K) & 1u;
+    const float f = boundary_phase<float, CBC>(chi, scale, cross, bc.re[MU], FWD ? bc.im[MU] : -bc.im[MU]);
+    reconstruct_accumulate<float, MU, FWD ? +1 : -1>(acc, chi, f);
+}
+
+// 16-bit storage: 2 = arithmetic on the stored f16 operands (above); 1 = exact projection with mixed-precision adds, the
+// rest in f32 after conversion; 0 = convert all 24 components and the link first
 #ifndef LQCD_F16_MIXED
-#define LQCD_F16_MIXED 1
+#define LQCD_F16_MIXED 2
 #endif
 
 // Hop K = 2 mu + (backward ? 1 : 0): gather the neighbour spinor and the link stored for this hop
@@ -184,6 +300,10 @@ __device__ __forceinline__ void hop_step(typename Compute<S>::type acc[24],
     using R = typename Compute<S>::type;
     constexpr int MU = K / 2;
     constexpr bool FWD = (K & 1) == 0;
+    if constexpr (sizeof(S) == 2 && LQCD_F16_MIXED == 2) {
+        hop_step_hh<CBC, K>(acc, site_links, in, ntiles, nb, crossmask, bc);
+        return;
+    }
     R h[12], u[18], scale;
     if constexpr (sizeof(S) == 2 && LQCD_F16_MIXED) {
         uint4 w[3];
@@ -262,7 +382,7 @@ __device__ __forceinline__ void hops_x_shuffled(R acc[24], const typename LinkSt
 #define LQCD_MINB_F64_R18 4
 #endif
 #ifndef LQCD_MINB_F16_R12
-#define LQCD_MINB_F16_R12 8
+#define LQCD_MINB_F16_R12 10
 #endif
 #ifndef LQCD_MINB_F32_R8
 #define LQCD_MINB_F32_R8 8

@@ -287,6 +287,18 @@ __device__ __forceinline__ void load_spinor_h(const __half* __restrict__ base, i
         unpack_h8(w, v + 8 * q);
     }
 }
+// the same with coherent loads, for a field the calling kernel also writes (p of the CG update)
+__device__ __forceinline__ void load_spinor_h_rw(const __half* base, int ntiles, int cb, float v[24], float& n) {
+    const uint4* words = reinterpret_cast<const uint4*>(base);
+    const uint4* p = words + (size_t)(cb / TILE) * (HALF_Q * TILE) + (cb % TILE);
+    asm volatile("ld.global.f32 %0, [%1];" : "=f"(n) : "l"(reinterpret_cast<const float*>(words + half_spinor_words(ntiles)) + cb) : "memory");
+#pragma unroll
+    for (int q = 0; q < HALF_Q; ++q) {
+        uint4 w;
+        asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "l"(p + q * TILE) : "memory");
+        unpack_h8(w, v + 8 * q);
+    }
+}
 
 // the stored words themselves (for the mixed-precision projection of dslash_kernel.cuh) and the site norm
 __device__ __forceinline__ void load_words_h(const __half* __restrict__ base, int ntiles, int cb, uint4 w[3], float& n) {

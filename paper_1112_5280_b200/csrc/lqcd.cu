@@ -7,6 +7,7 @@
 #include <cstdint>
 #include <cstring>
 #include <new>
+#include <type_traits>
 
 #include "blas_kernels.cuh"
 #include "pack_kernels.cuh"
@@ -367,21 +368,30 @@ struct CgWorkspace {
     int nblk;
 };
 
+// native half spinor of precision `prec` on the lattice of c (bytes, padded to whole tiles)
+inline size_t half_bytes_of(const lqcd_ctx* c, int prec) {
+    return (size_t)TILE * c->g.ntiles * (prec == 16 ? 24 * 2 + 4 : 24 * (prec / 8));
+}
+// storage precision of the CG iterate and residual for an operator context: 16-bit operators iterate with fp32 x and r
+inline int cg_x_precision(const lqcd_ctx* c) { return c->p.precision == 16 ? 32 : c->p.precision; }
+
+// r in the iterate's format; p, t = Q p, s = A p and the operator's intermediate in the operator's format
 CgWorkspace carve_cg(const lqcd_ctx* c, void* ws) {
     CgWorkspace w;
-    const size_t hb = align256(half_bytes(c));
+    const size_t hx = align256(half_bytes_of(c, cg_x_precision(c))), hp = align256(half_bytes(c));
     char* base = static_cast<char*>(ws);
-    w.r = base; w.p = base + hb; w.t = base + 2 * hb; w.s = base + 3 * hb; w.tmp = base + 4 * hb;
+    w.r = base; w.p = base + hx; w.t = w.p + hp; w.s = w.t + hp; w.tmp = w.s + hp;
     w.nblk = (c->g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
-    w.partial = reinterpret_cast<double*>(base + 5 * hb);
-    w.sc = reinterpret_cast<CgScalars*>(base + 5 * hb + align256((size_t)w.nblk * sizeof(double)));
+    w.partial = reinterpret_cast<double*>(w.tmp + hp);
+    w.sc = reinterpret_cast<CgScalars*>(w.tmp + hp + align256((size_t)w.nblk * sizeof(double)));
     return w;
 }
 
-template <typename R>
+// X: storage type of x, b, r;  P: storage type of the operator context c (p, Q p, A p)
+template <typename X, typename P>
 lqcd_status cg_loop(const lqcd_ctx* c, void* x, const void* gauge, const void* b, double kappa, double mu, double tol,
                     int maxiter, const CgWorkspace& w, int* iters_out, double* relres_out, cudaStream_t st) {
-    const size_t hb = half_bytes(c);
+    const size_t hx = half_bytes_of(c, cg_x_precision(c));
     const double theta = 2.0 * kappa * mu;
     const Geom& g = c->g;
     cudaError_t e;
@@ -390,10 +400,15 @@ lqcd_status cg_loop(const lqcd_ctx* c, void* x, const void* gauge, const void* b
     CgScalars init{};
     init.tol2 = tol * tol;
     if ((e = cudaMemcpyAsync(w.sc, &init, sizeof(init), cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
-    if ((e = cudaMemsetAsync(x, 0, hb, st)) != cudaSuccess) return cuda_fail(e);
-    if ((e = cudaMemcpyAsync(w.r, b, hb, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return cuda_fail(e);
-    if ((e = cudaMemcpyAsync(w.p, b, hb, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return cuda_fail(e);
-    norm2_kernel<R><<<w.nblk, BLAS_BLOCK, 0, st>>>((const R*)b, g, w.partial);
+    if ((e = cudaMemsetAsync(x, 0, hx, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(w.r, b, hx, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if constexpr (std::is_same<X, P>::value) {
+        if ((e = cudaMemcpyAsync(w.p, b, hx, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    } else {
+        convert_kernel<P, X><<<w.nblk, BLAS_BLOCK, 0, st>>>((P*)w.p, (const X*)b, g);
+        if ((s = after_launch()) != LQCD_OK) return s;
+    }
+    norm2_kernel<X><<<w.nblk, BLAS_BLOCK, 0, st>>>((const X*)b, g, w.partial);
     if ((s = after_launch()) != LQCD_OK) return s;
     cg_scalar_kernel<<<1, BLAS_BLOCK, 0, st>>>(w.partial, w.nblk, w.sc, CG_OP_INIT);
     if ((s = after_launch()) != LQCD_OK) return s;
@@ -409,17 +424,17 @@ lqcd_status cg_loop(const lqcd_ctx* c, void* x, const void* gauge, const void* b
         for (int k = 0; k < chunk; ++k) {
             // t = Q(mu) p ; alpha = rr / |t|^2
             if ((s = apply_M_impl(c, w.t, gauge, w.p, kappa, theta, true, 1, w.tmp, st, 1)) != LQCD_OK) return s;
-            norm2_kernel<R><<<w.nblk, BLAS_BLOCK, 0, st>>>((const R*)w.t, g, w.partial);
+            norm2_kernel<P><<<w.nblk, BLAS_BLOCK, 0, st>>>((const P*)w.t, g, w.partial);
             if ((s = after_launch()) != LQCD_OK) return s;
             cg_scalar_kernel<<<1, BLAS_BLOCK, 0, st>>>(w.partial, w.nblk, w.sc, CG_OP_PAP);
             if ((s = after_launch()) != LQCD_OK) return s;
             // s = Q(-mu) t = A p ; x += alpha p ; r -= alpha s ; rr', beta, convergence
             if ((s = apply_M_impl(c, w.s, gauge, w.t, kappa, -theta, true, 1, w.tmp, st, 1)) != LQCD_OK) return s;
-            cg_update_xr_kernel<R><<<w.nblk, BLAS_BLOCK, 0, st>>>((R*)x, (R*)w.r, (const R*)w.p, (const R*)w.s, g, w.sc, w.partial);
+            cg_update_xr_kernel<X, P><<<w.nblk, BLAS_BLOCK, 0, st>>>((X*)x, (X*)w.r, (const P*)w.p, (const P*)w.s, g, w.sc, w.partial);
             if ((s = after_launch()) != LQCD_OK) return s;
             cg_scalar_kernel<<<1, BLAS_BLOCK, 0, st>>>(w.partial, w.nblk, w.sc, CG_OP_RR);
             if ((s = after_launch()) != LQCD_OK) return s;
-            cg_update_p_kernel<R><<<w.nblk, BLAS_BLOCK, 0, st>>>((R*)w.p, (const R*)w.r, g, w.sc);
+            cg_update_p_kernel<X, P><<<w.nblk, BLAS_BLOCK, 0, st>>>((P*)w.p, (const X*)w.r, g, w.sc);
             if ((s = after_launch()) != LQCD_OK) return s;
         }
         it += chunk;
@@ -455,10 +470,17 @@ lqcd_status norm2_to_host(const lqcd_ctx* c, const void* v, double* partial, dou
 
 extern "C" {
 
+// the loop's own scratch (carve_cg)
+static size_t cg_loop_bytes(const lqcd_ctx* c) {
+    const int nblk = (c->g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
+    return align256(half_bytes_of(c, cg_x_precision(c))) + 4 * align256(half_bytes(c)) + align256((size_t)nblk * sizeof(double)) +
+           align256(sizeof(CgScalars));
+}
+
 size_t lqcd_cg_workspace_bytes(const lqcd_ctx* c) {
     if (!c) return 0;
-    const int nblk = (c->g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
-    return 5 * align256(half_bytes(c)) + align256((size_t)nblk * sizeof(double)) + align256(sizeof(CgScalars));
+    // a 16-bit context iterates on fp32 copies of b and x: two more fp32 half spinors
+    return cg_loop_bytes(c) + (c->p.precision == 16 ? 2 * align256(half_bytes_of(c, 32)) : 0);
 }
 
 lqcd_status lqcd_apply_Q_tm(const lqcd_ctx* c, void* out, const void* gauge, const void* in, double kappa, double mu,
@@ -471,15 +493,29 @@ lqcd_status lqcd_cg_solve_tm(const lqcd_ctx* c, void* x, const void* gauge, cons
     const size_t hb = c ? half_bytes(c) : 0;
     lqcd_status s = check_fields(c, x, gauge, b, hb);
     if (s != LQCD_OK) return s;
-    if (c->p.precision == 16) return LQCD_EUNSUPPORTED;  // the solver's vectors are fp32 / fp64
     if (!workspace || !(tol > 0.0) || maxiter < 0) return LQCD_EINVAL;
     if (reinterpret_cast<uintptr_t>(workspace) & 255u) return LQCD_EALIGN;
     const size_t wb = lqcd_cg_workspace_bytes(c);
     if (overlaps(workspace, wb, x, hb) || overlaps(workspace, wb, b, hb)) return LQCD_EALIAS;
-    const CgWorkspace w = carve_cg(c, workspace);
     cudaStream_t st = (cudaStream_t)stream;
-    return c->p.precision == 32 ? cg_loop<float>(c, x, gauge, b, kappa, mu, tol, maxiter, w, iters_out, relres_out, st)
-                                : cg_loop<double>(c, x, gauge, b, kappa, mu, tol, maxiter, w, iters_out, relres_out, st);
+    if (c->p.precision == 16) {
+        // 16-bit storage: the iterate and the residual live in fp32 (their recurrences carry the accuracy), the search
+        // direction and the operator's vectors in the 16-bit format; b is widened first, x rounded to storage at the end
+        char* b32 = static_cast<char*>(workspace);
+        char* x32 = b32 + align256(half_bytes_of(c, 32));
+        const CgWorkspace w = carve_cg(c, x32 + align256(half_bytes_of(c, 32)));
+        convert_kernel<float, __half><<<w.nblk, BLAS_BLOCK, 0, st>>>((float*)b32, (const __half*)b, c->g);
+        if ((s = after_launch()) != LQCD_OK) return s;
+        s = cg_loop<float, __half>(c, x32, gauge, b32, kappa, mu, tol, maxiter, w, iters_out, relres_out, st);
+        if (s != LQCD_OK) return s;
+        convert_kernel<__half, float><<<w.nblk, BLAS_BLOCK, 0, st>>>((__half*)x, (const float*)x32, c->g);
+        if ((s = after_launch()) != LQCD_OK) return s;
+        const cudaError_t e = cudaStreamSynchronize(st);
+        return e == cudaSuccess ? LQCD_OK : cuda_fail(e);
+    }
+    const CgWorkspace w = carve_cg(c, workspace);
+    return c->p.precision == 32 ? cg_loop<float, float>(c, x, gauge, b, kappa, mu, tol, maxiter, w, iters_out, relres_out, st)
+                                : cg_loop<double, double>(c, x, gauge, b, kappa, mu, tol, maxiter, w, iters_out, relres_out, st);
 }
 
 // Mixed precision: fp64 defect correction around the fp32 CG (reading F2).
@@ -488,7 +524,7 @@ lqcd_status lqcd_cg_solve_tm(const lqcd_ctx* c, void* x, const void* gauge, cons
 size_t lqcd_cg_mixed_workspace_bytes(const lqcd_ctx* c64, const lqcd_ctx* c32) {
     if (!c64 || !c32) return 0;
     const int nblk = (c64->g.Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
-    return 4 * align256(half_bytes(c64)) + 2 * align256(half_bytes(c32)) + align256(lqcd_cg_workspace_bytes(c32)) +
+    return 4 * align256(half_bytes(c64)) + 2 * align256(half_bytes_of(c32, 32)) + align256(cg_loop_bytes(c32)) +
            align256((size_t)nblk * sizeof(double)) + 256;
 }
 
@@ -497,11 +533,11 @@ lqcd_status lqcd_cg_solve_tm_mixed(const lqcd_ctx* c64, const lqcd_ctx* c32, voi
                                    double inner_tol, int maxiter, void* workspace, int* iters_out, int* outer_out,
                                    double* relres_out, void* stream) {
     if (!c64 || !c32 || !gauge32) return LQCD_EINVAL;
-    if (c64->p.precision != 64 || c32->p.precision != 32) return LQCD_EINVAL;
+    if (c64->p.precision != 64 || (c32->p.precision != 32 && c32->p.precision != 16)) return LQCD_EINVAL;
     for (int m = 0; m < 4; ++m)
         if (c64->p.dims[m] != c32->p.dims[m] || c64->p.bc_re[m] != c32->p.bc_re[m] || c64->p.bc_im[m] != c32->p.bc_im[m])
             return LQCD_EINVAL;
-    const size_t hb64 = half_bytes(c64), hb32 = half_bytes(c32);
+    const size_t hb64 = half_bytes(c64), hb32 = half_bytes_of(c32, 32);   // the inner iterate and residual are fp32 also for a 16-bit inner operator
     lqcd_status s = check_fields(c64, x, gauge64, b, hb64);
     if (s != LQCD_OK) return s;
     if (!workspace || !(tol > 0.0) || !(inner_tol > 0.0) || maxiter < 0) return LQCD_EINVAL;
@@ -520,7 +556,7 @@ lqcd_status lqcd_cg_solve_tm_mixed(const lqcd_ctx* c64, const lqcd_ctx* c32, voi
     char* tmp64 = base;                 base += align256(hb64);
     char* r32 = base;                   base += align256(hb32);
     char* e32 = base;                   base += align256(hb32);
-    char* inner_ws = base;              base += align256(lqcd_cg_workspace_bytes(c32));
+    char* inner_ws = base;              base += align256(cg_loop_bytes(c32));
     double* partial = reinterpret_cast<double*>(base);  base += align256((size_t)nblk * sizeof(double));
     double* scratch = reinterpret_cast<double*>(base);
     const CgWorkspace iw = carve_cg(c32, inner_ws);
@@ -539,8 +575,9 @@ lqcd_status lqcd_cg_solve_tm_mixed(const lqcd_ctx* c64, const lqcd_ctx* c32, voi
         if ((s = after_launch()) != LQCD_OK) return s;
         const double need = tol * std::sqrt(bb / rr);  // relative reduction of |r| still required
         int it = 0;
-        s = cg_loop<float>(c32, e32, gauge32, r32, kappa, mu, inner_tol > 0.5 * need ? inner_tol : 0.5 * need,
-                           maxiter - total, iw, &it, nullptr, st);
+        const double itol = inner_tol > 0.5 * need ? inner_tol : 0.5 * need;
+        s = c32->p.precision == 16 ? cg_loop<float, __half>(c32, e32, gauge32, r32, kappa, mu, itol, maxiter - total, iw, &it, nullptr, st)
+                                   : cg_loop<float, float>(c32, e32, gauge32, r32, kappa, mu, itol, maxiter - total, iw, &it, nullptr, st);
         if (s != LQCD_OK) return s;
         total += it;
         ++outer;

@@ -108,3 +108,54 @@ def test_mixed_precision_cg(recon64, recon32, link32):
     import paper_1112_5280_b200 as L
     with pytest.raises(L.LqcdError):
         g32.ctx.cg_solve_tm_mixed(g64.ctx, x, g64.gauge, g32.gauge, g64.buf(), kappa, mu, tol, 1e-4, 10, ws)
+
+
+def test_mixed_precision_cg_16bit_inner():
+    """lqcd_cg_solve_tm_mixed with a precision-16 inner context (16-bit solver, next row f4): the inner CG keeps x and r
+    in fp32 and p, Q p, A p in 16-bit storage; the fp64 defect correction restores full accuracy.  Checked like the fp32
+    inner solver: true residual with the oracle's operator, solution against the fp64 oracle CG; the iteration count
+    may exceed the fp32-inner model of the oracle (a 2^-11 perturbed operator and search direction), bounded at 2x."""
+    import gpu_harness as H
+    dims, kappa, mu, tol = (8, 8, 8, 16), 0.15, 0.1, 1e-11
+    U = li.links_for_config(2)
+    even = li.parity_mask(dims, 0)[..., None, None]
+    b = li.gaussian_spinor(dims, seed=41) * even
+    g64 = H.Gpu(dims, 64, 12, APBC, U)
+    g16 = H.Gpu(dims, 16, 12, APBC, U.astype(np.complex64))
+    x = g64.buf()
+    ws = torch.empty(g64.ctx.cg_mixed_workspace_bytes(g16.ctx), dtype=torch.uint8, device=g64.dev)
+    it, outer, res = g64.ctx.cg_solve_tm_mixed(g16.ctx, x, g64.gauge, g16.gauge, g64.to_native(H.half_of(b, dims, 0), 0),
+                                               kappa, mu, tol, 1e-3, 4000, ws)
+    xg = H.scatter_half(g64.from_native(x, 0), dims, 0)
+    Ax = G5 * oracle.apply_M_tm(U, G5 * oracle.apply_M_tm(U, xg, dims, APBC, kappa, mu, 1), dims, APBC, kappa, -mu, 1)
+    assert res <= tol and np.linalg.norm(b - Ax) <= 1.5 * tol * np.linalg.norm(b)
+    x_ref, it_ref, _ = cg_oracle.cg_solve_tm(U, b, dims, APBC, kappa, mu, tol, 500)
+    assert np.linalg.norm(xg - x_ref) <= 100 * tol * np.linalg.norm(x_ref)
+    _, it_mix, outer_mix, _ = cg_oracle.cg_mixed_solve_tm(U, b, dims, APBC, kappa, mu, tol, 1e-3, 4000)
+    assert it <= 2 * it_mix + 10 and outer <= 2 * outer_mix + 4, (it, it_mix, outer, outer_mix)
+
+
+def test_cg_16bit_context():
+    """lqcd_cg_solve_tm on a precision-16 context: 16-bit b in, 16-bit x out, fp32 iterate inside.  The operator it
+    inverts is the one on the stored (rounded) links; against the oracle on those links the solution is good to the
+    storage rounding of x (2^-11 per site) plus cond(A) times the 16-bit noise of the recurrences."""
+    import gpu_harness as H
+    import test_gpu_parity as T
+    dims, kappa, mu, tol = (8, 8, 8, 16), 0.15, 0.1, 2e-3
+    U = li.links_for_config(2).astype(np.complex64)
+    even = li.parity_mask(dims, 0)[..., None, None]
+    b = (li.gaussian_spinor(dims, seed=43) * even).astype(np.complex64)
+    g = H.Gpu(dims, 16, 12, APBC, U)
+    ws = torch.empty(g.ctx.cg_workspace_bytes(), dtype=torch.uint8, device=g.dev)
+    x = g.buf()
+    it, res = g.ctx.cg_solve_tm(x, g.gauge, g.to_native(H.half_of(b, dims, 0), 0), kappa, mu, tol, 500, ws)
+    assert 0 < it < 100 and res <= tol
+    Uq, bq = T._quantise_links(U), T._quantise_spinor(b)
+    xg = H.scatter_half(g.from_native(x, 0), dims, 0)
+    Ax = G5 * oracle.apply_M_tm(Uq, G5 * oracle.apply_M_tm(Uq, xg, dims, APBC, kappa, mu, 1), dims, APBC, kappa, -mu, 1)
+    assert np.linalg.norm(bq - Ax) <= 5 * tol * np.linalg.norm(bq)
+    # zero source, and the iteration cut-off
+    it0, res0 = g.ctx.cg_solve_tm(x, g.gauge, g.to_native(np.zeros_like(H.half_of(b, dims, 0)), 0), kappa, mu, tol, 50, ws)
+    assert it0 == 0 and res0 == 0.0 and not g.from_native(x, 0).any()
+    it3, _ = g.ctx.cg_solve_tm(x, g.gauge, g.to_native(H.half_of(b, dims, 0), 0), kappa, mu, 1e-9, 3, ws)
+    assert it3 == 3

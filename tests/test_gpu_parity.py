@@ -299,23 +299,23 @@ def test_half_precision_storage(H, dims, bc):
         got = g.dslash_eo(H.half_of(psi, dims, 1 - op), op)
         ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, op), dims, op)
         assert H.rel_l2(got, ref) <= TOL16
-        # against the oracle fed the values actually stored: only the output rounding (2^-11 of the site max) is left
+        # against the oracle fed the values actually stored (reading F4): left are the output rounding
+        # (2^-11 of the site max: 1.8e-4) and the two f16 roundings per hop of the arithmetic on stored operands -- the
+        # projected half spinor (rms 2^-11 x 0.42 = 2.0e-4 of each component) and the rebuilt third link row (the same on a
+        # third of the link entries: 1.2e-4): 3.0e-4 in quadrature, bar at twice that
         refq = H.half_of(oracle.dslash_eo(Uq, psiq, dims, bc, op), dims, op)
         assert H.rel_l2(got, refq) <= 6e-4
-        assert H.rel_l2(got, _quantise_spinor(refq.astype(np.complex64))) <= 2e-4   # up to ties at rounding boundaries
+        # both sides on the output grid: the arithmetic part alone (2.3e-4) plus grid points it flips; same bar
+        assert H.rel_l2(got, _quantise_spinor(refq.astype(np.complex64))) <= 6e-4
     assert H.rel_l2(g.dslash_full(psi), oracle.dslash_full(U, psi, dims, bc)) <= TOL16
     refM = H.half_of(oracle.apply_M(U, psi, dims, bc, 0.15, 1), dims, 0)
     assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), 0.15, 1), refM) <= TOL16
     refT = H.half_of(oracle.apply_M_tm(U, psi, dims, bc, 0.15, 0.3, 1), dims, 0)
     assert H.rel_l2(g.apply_M(H.half_of(psi, dims, 0), 0.15, 1, mu=0.3), refT) <= TOL16
     assert H.rel_l2(g.apply_M(psi, 0.15, 0, mu=-0.2), oracle.apply_M_tm(U, psi, dims, bc, 0.15, -0.2, 0)) <= TOL16
-    # a zero site stays zero (norm 0), and the solver entry points refuse 16-bit contexts
+    # a zero site stays zero (norm 0)
     z = np.zeros_like(H.half_of(psi, dims, 1))
     assert not g.dslash_eo(z, 0).any()
-    import torch, paper_1112_5280_b200 as L
-    with pytest.raises(L.LqcdError) as e:
-        g.ctx.cg_solve_tm(g.buf(), g.gauge, g.buf(), 0.1, 0.1, 1e-3, 5, torch.empty(1 << 20, dtype=torch.uint8, device="cuda:0"))
-    assert e.value.status == L.LQCD_EUNSUPPORTED
 
 
 @pytest.mark.parametrize("precision", [16, 32, 64])
