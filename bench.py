@@ -49,7 +49,7 @@ NOMINAL_HBM_GBS = 8000.0              # north_star's "~8 TB/s"
 MIN_REGION_LAUNCHES = 200
 MIN_REGION_MS = 100.0
 SUSTAINED_S = 1.5
-ALL_LEGS = ("fp64", "recon18", "recon8", "matrix", "cg", "cgmixed", "fp16", "config3", "chain", "e2e", "slab", "cpu")
+ALL_LEGS = ("fp64", "recon18", "recon8", "matrix", "cg", "cgmixed", "fp16", "config3", "chain", "e2e", "slab", "heatbath", "cpu")
 
 
 def parse_args():
@@ -566,6 +566,44 @@ def cg_mixed_leg(torch, w64, w32, mu=0.05, tol=1e-10, inner_tol=1e-4, maxiter=20
             "ms": best}
 
 
+def heatbath_leg(torch, dev, cfg_id=4, beta=6.0, ntries=4, sweeps=3):
+    """Next row f4, last clause: pure-gauge SU(3) heatbath sweeps (8 sublattice launches each) on the config's lattice,
+    fp64, canonical link field, uniforms drawn on the device beforehand (they are inputs of the method).  Bytes per link
+    update (model): the 18 staple links and the link itself are shared with other updates -- each launch touches all
+    links of the three other directions (3 V), the mu links of both parities (V) and writes V/2: 9 links of 144 B per
+    update -- plus the uniforms of one attempt and the direction per subgroup (3 x 6 x 8 B)."""
+    import numpy as np
+    import lattice_inputs as li
+    import paper_1112_5280_b200 as L
+    c = li.CONFIGS[cfg_id]
+    ctx = L.Context(c["dims"], 64, 18, (1, 1, 1, 1))
+    U = torch.from_numpy(li.links_for_config(cfg_id, dtype=np.complex128)).to(dev)
+    ws = torch.empty(ctx.plaquette_workspace_bytes(), dtype=torch.uint8, device=dev)
+    p0 = ctx.plaquette(U, ws)
+    n = ctx.heatbath_uniforms(ntries)
+    u = [1.0 - torch.rand(n, dtype=torch.float64, device=dev) for _ in range(2)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    times = []
+    for s in range(sweeps + 1):
+        torch.cuda.synchronize()
+        e0.record()
+        for mu in range(4):
+            for parity in (0, 1):
+                ctx.heatbath_sublattice(U, beta, mu, parity, u[(mu + parity) & 1], ntries)
+        e1.record()
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1))
+        for t in u:
+            t.copy_(1.0 - torch.rand(n, dtype=torch.float64, device=dev))
+    ms = sorted(times[1:])[len(times[1:]) // 2]
+    links = 4 * 2 * ctx.Vh
+    nbytes = links * (9 * 144 + 3 * 6 * 8)
+    return {"workload": f"config {cfg_id} lattice {'x'.join(map(str, c['dims']))}, fp64, beta {beta}, {ntries} attempts per subgroup",
+            "ms_per_sweep": ms, "us_per_sublattice_launch": ms * 1e3 / 8, "link_updates_per_s": links / (ms * 1e-3),
+            "gbs_model": nbytes / (ms * 1e-3) / 1e9, "bytes_per_link_update_model": 9 * 144 + 144,
+            "plaquette_before": p0, "plaquette_after": ctx.plaquette(U, ws), "sweeps_timed": sweeps}
+
+
 def cpu_baseline_leg(cfg_id, precision):
     """The oracle as it stands on the host cores: full-lattice dslash_eo of the same workload,
     one warm-up then best of 3 (about 2-5 s of CPU work on 8+ cores)."""
@@ -755,6 +793,8 @@ def run_b200(args):
             line["chain"] = [chain_leg(torch, 5, 32, rc, dev, U=U5, kernel=args.kernel) for rc in (12, 18)]
             line["chain_link_generation_s"] = gen_s
             del U5
+        if want("heatbath"):
+            line["heatbath"] = heatbath_leg(torch, dev, args.config)
         if want("cpu"):
             line["cpu_baseline"] = cpu_baseline_leg(args.config, 32 if args.precision == 16 else args.precision)
     sampler.close()

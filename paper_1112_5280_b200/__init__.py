@@ -21,7 +21,8 @@ EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
     "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_set_time_slab", "lqcd_dslash_eo_range", "lqcd_pack_gauge_slab", "lqcd_halo_bytes", "lqcd_slab_push_faces", "lqcd_dslash_eo_slab", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_dslash_eo_host_batch", "lqcd_launch_count",
-    "lqcd_gauge_recon8_margin", "lqcd_set_kernel", "lqcd_status_string", "lqcd_last_cuda_error",
+    "lqcd_gauge_recon8_margin", "lqcd_set_kernel", "lqcd_heatbath_uniforms", "lqcd_heatbath_sublattice",
+    "lqcd_plaquette_workspace_bytes", "lqcd_plaquette", "lqcd_status_string", "lqcd_last_cuda_error",
 ]
 
 
@@ -66,6 +67,12 @@ def _lib():
         lib.lqcd_apply_M.argtypes = [vp, vp, vp, vp, cd, ci, vp, vp]
         lib.lqcd_set_time_slab.argtypes = [vp, ci, ci]
         lib.lqcd_set_kernel.argtypes = [vp, ci]
+        lib.lqcd_heatbath_uniforms.argtypes = [vp, ci]
+        lib.lqcd_heatbath_uniforms.restype = sz
+        lib.lqcd_heatbath_sublattice.argtypes = [vp, vp, cd, ci, ci, vp, ci, vp]
+        lib.lqcd_plaquette_workspace_bytes.argtypes = [vp]
+        lib.lqcd_plaquette_workspace_bytes.restype = sz
+        lib.lqcd_plaquette.argtypes = [vp, vp, vp, ctypes.POINTER(cd), vp]
         lib.lqcd_dslash_eo_range.argtypes = [vp, vp, vp, vp, ci, ci, ci, vp]
         lib.lqcd_halo_bytes.argtypes = [vp]
         lib.lqcd_halo_bytes.restype = sz
@@ -167,6 +174,20 @@ class Context:
     def dslash_eo(self, out, gauge, inp, out_parity, stream=None):
         _chk(_lib().lqcd_dslash_eo(self._h, _ptr(out), _ptr(gauge), _ptr(inp), int(out_parity), _stream(stream)),
              "lqcd_dslash_eo")
+
+    # pure-gauge heatbath (canonical complex128 link field, in place)
+    def heatbath_uniforms(self, ntries): return _lib().lqcd_heatbath_uniforms(self._h, int(ntries))
+
+    def heatbath_sublattice(self, links, beta, mu, parity, uniforms, ntries, stream=None):
+        _chk(_lib().lqcd_heatbath_sublattice(self._h, _ptr(links), float(beta), int(mu), int(parity), _ptr(uniforms),
+                                             int(ntries), _stream(stream)), "lqcd_heatbath_sublattice")
+
+    def plaquette_workspace_bytes(self): return _lib().lqcd_plaquette_workspace_bytes(self._h)
+
+    def plaquette(self, links, workspace, stream=None):
+        p = ctypes.c_double(0.0)
+        _chk(_lib().lqcd_plaquette(self._h, _ptr(links), _ptr(workspace), ctypes.byref(p), _stream(stream)), "lqcd_plaquette")
+        return p.value
 
     def set_kernel(self, kernel):
         _chk(_lib().lqcd_set_kernel(self._h, int(kernel)), "lqcd_set_kernel")

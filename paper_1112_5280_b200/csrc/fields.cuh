@@ -92,14 +92,14 @@ __device__ __forceinline__ void stg256(double4_* p, const double* v) {
 template <typename R>
 __host__ __device__ __forceinline__ size_t spinor_word0(int cb) {
     constexpr int Q = 24 / Word<R>::W;
-    return (size_t)(cb / TILE) * (Q * TILE) + (cb % TILE);
+    return (size_t)((unsigned)cb / TILE) * (Q * TILE) + ((unsigned)cb % TILE);
 }
 
 // word 0 of hop k's link of site cb (parity p); word w is w * TILE words further on
 template <typename R, int RECON>
 __host__ __device__ __forceinline__ size_t link_word0(int ntiles, int p, int cb, int k) {
     constexpr int NW = RECON / LinkWord<R, RECON>::LW;
-    return ((size_t)(p * ntiles + cb / TILE) * 8 + k) * (NW * TILE) + (cb % TILE);
+    return ((size_t)(p * ntiles + (int)((unsigned)cb / TILE)) * 8 + k) * (NW * TILE) + ((unsigned)cb % TILE);
 }
 
 // Spinor loads go through the read-only path (ld.global.nc) with default caching: each input spinor is gathered
@@ -279,7 +279,7 @@ __device__ __forceinline__ void unpack_h8(const uint4& w, float* v) {
 // forms n * v: the hop is linear, so n rides on the accumulation factor of step K5.
 __device__ __forceinline__ void load_spinor_h(const __half* __restrict__ base, int ntiles, int cb, float v[24], float& n) {
     const uint4* words = reinterpret_cast<const uint4*>(base);
-    const uint4* p = words + (size_t)(cb / TILE) * (HALF_Q * TILE) + (cb % TILE);
+    const uint4* p = words + (size_t)((unsigned)cb / TILE) * (HALF_Q * TILE) + ((unsigned)cb % TILE);
     n = __ldg(reinterpret_cast<const float*>(words + half_spinor_words(ntiles)) + cb);
 #pragma unroll
     for (int q = 0; q < HALF_Q; ++q) {
@@ -290,7 +290,7 @@ __device__ __forceinline__ void load_spinor_h(const __half* __restrict__ base, i
 // the same with coherent loads, for a field the calling kernel also writes (p of the CG update)
 __device__ __forceinline__ void load_spinor_h_rw(const __half* base, int ntiles, int cb, float v[24], float& n) {
     const uint4* words = reinterpret_cast<const uint4*>(base);
-    const uint4* p = words + (size_t)(cb / TILE) * (HALF_Q * TILE) + (cb % TILE);
+    const uint4* p = words + (size_t)((unsigned)cb / TILE) * (HALF_Q * TILE) + ((unsigned)cb % TILE);
     asm volatile("ld.global.f32 %0, [%1];" : "=f"(n) : "l"(reinterpret_cast<const float*>(words + half_spinor_words(ntiles)) + cb) : "memory");
 #pragma unroll
     for (int q = 0; q < HALF_Q; ++q) {
@@ -303,7 +303,7 @@ __device__ __forceinline__ void load_spinor_h_rw(const __half* base, int ntiles,
 // the stored words themselves (for the mixed-precision projection of dslash_kernel.cuh) and the site norm
 __device__ __forceinline__ void load_words_h(const __half* __restrict__ base, int ntiles, int cb, uint4 w[3], float& n) {
     const uint4* words = reinterpret_cast<const uint4*>(base);
-    const uint4* p = words + (size_t)(cb / TILE) * (HALF_Q * TILE) + (cb % TILE);
+    const uint4* p = words + (size_t)((unsigned)cb / TILE) * (HALF_Q * TILE) + ((unsigned)cb % TILE);
     n = __ldg(reinterpret_cast<const float*>(words + half_spinor_words(ntiles)) + cb);
 #pragma unroll
     for (int q = 0; q < HALF_Q; ++q) w[q] = __ldg(p + q * TILE);
@@ -311,7 +311,7 @@ __device__ __forceinline__ void load_words_h(const __half* __restrict__ base, in
 
 __device__ __forceinline__ void store_spinor_h(__half* __restrict__ base, int ntiles, int cb, const float v[24]) {
     uint4* words = reinterpret_cast<uint4*>(base);
-    uint4* p = words + (size_t)(cb / TILE) * (HALF_Q * TILE) + (cb % TILE);
+    uint4* p = words + (size_t)((unsigned)cb / TILE) * (HALF_Q * TILE) + ((unsigned)cb % TILE);
     float n = 0.f;
 #pragma unroll
     for (int k = 0; k < 24; ++k) n = fmaxf(n, fabsf(v[k]));
@@ -329,7 +329,7 @@ __device__ __forceinline__ void store_spinor_h(__half* __restrict__ base, int nt
 
 // word 0 of hop k's link of site cb (parity p) in the half-precision link field, in 8-byte words
 __host__ __device__ __forceinline__ size_t link_word0_h(int ntiles, int p, int cb, int k) {
-    return ((size_t)(p * ntiles + cb / TILE) * 8 + k) * (3 * TILE) + (cb % TILE);
+    return ((size_t)(p * ntiles + (int)((unsigned)cb / TILE)) * 8 + k) * (3 * TILE) + ((unsigned)cb % TILE);
 }
 
 __device__ __forceinline__ void load_link_h(const uint2* __restrict__ site_links, int k, float u[18]) {

@@ -10,6 +10,7 @@
 #include <type_traits>
 
 #include "blas_kernels.cuh"
+#include "heatbath_kernels.cuh"
 #include "pack_kernels.cuh"
 #include "slab_launch.cuh"
 
@@ -687,6 +688,48 @@ lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* c, void* out_host, const void* g
     void* outs[1] = {out_host};
     const void* ins[1] = {in_host};
     return lqcd_dslash_eo_host_batch(c, 1, outs, gauge_host, ins, &out_parity, ws, stream);
+}
+
+// ---- next row f4, last clause: pure-gauge heatbath on the canonical link field (heatbath_kernels.cuh) -------------------
+size_t lqcd_heatbath_uniforms(const lqcd_ctx* c, int ntries) {
+    return c && ntries > 0 ? (size_t)c->g.Vh * 3 * (4 * (size_t)ntries + 2) : 0;
+}
+
+lqcd_status lqcd_heatbath_sublattice(const lqcd_ctx* c, void* links, double beta, int mu, int parity, const void* uniforms,
+                                     int ntries, void* stream) {
+    if (!c || !links || !uniforms) return LQCD_EINVAL;
+    if (mu < 0 || mu > 3 || (parity != 0 && parity != 1) || ntries < 1 || ntries > 64 || !(beta > 0.0)) return LQCD_EINVAL;
+    if (c->p.precision != 64) return LQCD_EUNSUPPORTED;   // the canonical field of a precision-64 context (complex128)
+    if (!aligned16(links) || (reinterpret_cast<uintptr_t>(uniforms) & 7u)) return LQCD_EALIGN;
+    heatbath_kernel<<<(c->g.Vh + HB_BLOCK - 1) / HB_BLOCK, HB_BLOCK, 0, (cudaStream_t)stream>>>(
+        (double*)links, c->g, beta, mu, parity, (const double*)uniforms, ntries);
+    return after_launch();
+}
+
+size_t lqcd_plaquette_workspace_bytes(const lqcd_ctx* c) {
+    return c ? align256((size_t)((2 * (size_t)c->g.Vh + HB_BLOCK - 1) / HB_BLOCK) * sizeof(double)) + 256 : 0;
+}
+
+lqcd_status lqcd_plaquette(const lqcd_ctx* c, const void* links, void* workspace, double* plaq_host, void* stream) {
+    if (!c || !links || !workspace || !plaq_host) return LQCD_EINVAL;
+    if (c->p.precision != 64) return LQCD_EUNSUPPORTED;
+    if (!aligned16(links) || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return LQCD_EALIGN;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t V = 2 * (size_t)c->g.Vh;
+    const int nblk = (int)((V + HB_BLOCK - 1) / HB_BLOCK);
+    double* partial = static_cast<double*>(workspace);
+    double* total = reinterpret_cast<double*>(static_cast<char*>(workspace) + align256((size_t)nblk * sizeof(double)));
+    plaquette_kernel<<<nblk, HB_BLOCK, 0, st>>>((const double*)links, c->g, partial);
+    lqcd_status s = after_launch();
+    if (s != LQCD_OK) return s;
+    sum_partials_kernel<<<1, BLAS_BLOCK, 0, st>>>(partial, nblk, total);
+    if ((s = after_launch()) != LQCD_OK) return s;
+    double sum = 0.0;
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(&sum, total, sizeof(double), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+    *plaq_host = sum / (3.0 * 6.0 * (double)V);
+    return LQCD_OK;
 }
 
 unsigned long long lqcd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
