@@ -19,14 +19,20 @@
 namespace lqcd {
 
 constexpr int HB_BLOCK = 128;
+// resident blocks per SM promised to ptxas for the heatbath kernel (register budget 65536 / (128 x value))
+#ifndef LQCD_HB_MINB
+#define LQCD_HB_MINB 3
+#endif
 
 struct Mat3 { double re[9], im[9]; };   // row-major: element (r, c) at 3 r + c
 
-__device__ __forceinline__ void load_mat(const double* __restrict__ links, size_t link, Mat3& m) {
+// RO: the link is not written by the running launch (every link but the thread's own): read-only path
+template <bool RO = true>
+__device__ __forceinline__ void load_mat(const double* links, size_t link, Mat3& m) {
     const double2* p = reinterpret_cast<const double2*>(links) + link * 9;
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
-        const double2 z = p[k];
+        const double2 z = RO ? __ldg(p + k) : p[k];
         m.re[k] = z.x;
         m.im[k] = z.y;
     }
@@ -138,7 +144,7 @@ __device__ __forceinline__ Coords site_coords(const Geom& g, int cb, int parity)
 }
 
 // links: canonical [mu][V][3][3] complex128, updated in place for (mu, parity); uniforms: [V/2][3][4 ntries + 2]
-__global__ void __launch_bounds__(HB_BLOCK) heatbath_kernel(double* links, Geom g, double beta, int mu, int parity,
+__global__ void __launch_bounds__(HB_BLOCK, LQCD_HB_MINB) heatbath_kernel(double* links, Geom g, double beta, int mu, int parity,
                                                             const double* __restrict__ uniforms, int ntries) {
     const int cb = blockIdx.x * HB_BLOCK + threadIdx.x;
     if (cb >= g.Vh) return;
@@ -172,7 +178,7 @@ __global__ void __launch_bounds__(HB_BLOCK) heatbath_kernel(double* links, Geom 
         for (int k = 0; k < 9; ++k) { a.re[k] += q.re[k]; a.im[k] += q.im[k]; }
     }
     Mat3 u;
-    load_mat(links, mu * V + x0, u);
+    load_mat<false>(links, mu * V + x0, u);
     const double* r = uniforms + (size_t)cb * 3 * (4 * ntries + 2);
     subgroup_step<0, 1>(u, a, beta, r, ntries);
     subgroup_step<0, 2>(u, a, beta, r + (4 * ntries + 2), ntries);
