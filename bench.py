@@ -49,7 +49,7 @@ NOMINAL_HBM_GBS = 8000.0              # north_star's "~8 TB/s"
 MIN_REGION_LAUNCHES = 200
 MIN_REGION_MS = 100.0
 SUSTAINED_S = 1.5
-ALL_LEGS = ("fp64", "recon18", "recon8", "matrix", "cg", "cgmixed", "fp16", "config3", "chain", "e2e", "slab", "heatbath", "cpu")
+ALL_LEGS = ("fp64", "recon18", "recon8", "matrix", "cg", "cgmixed", "fp16", "config3", "chain", "e2e", "slab", "heatbath", "variants", "cpu")
 
 
 def parse_args():
@@ -61,7 +61,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="lattice_inputs.CONFIGS id of the main workload")
     ap.add_argument("--precision", type=int, default=32, choices=[16, 32, 64], help="precision of the primary line (16: half storage, fp32 arithmetic)")
     ap.add_argument("--recon", type=int, default=12, choices=[8, 12, 18])
-    ap.add_argument("--kernel", default="gather", choices=["gather", "pipe", "blocked"],
+    ap.add_argument("--kernel", default="gather", choices=["gather", "pipe", "blocked", "lstage"],
                     help="lqcd_set_kernel for the primary line and the fp64 / recon legs: gather (one thread per site) or pipe (TMA pipeline)")
     ap.add_argument("--no-extras", action="store_true", help="primary line only (profiling runs)")
     ap.add_argument("--legs", default="all", help="comma list of extra legs: " + ",".join(ALL_LEGS) + " (default all)")
@@ -194,6 +194,8 @@ class Workload:
             self.ctx.set_kernel(L.KERNEL_PIPE)
         if kernel == "blocked":
             self.ctx.set_kernel(L.KERNEL_BLOCKED)
+        if kernel == "lstage" and precision != 16 and not link_precision:
+            self.ctx.set_kernel(L.KERNEL_LSTAGE)
         self.kernel = kernel
         self.Vh = self.ctx.Vh
         if U is None:
@@ -750,6 +752,20 @@ def run_b200(args):
             del w16
     del w2
     torch.cuda.empty_cache()
+    if want("variants") and args.kernel == "gather" and args.precision != 16:
+        # the data-movement variants of the same arithmetic (lqcd_set_kernel), timed like the fp64 leg
+        line["kernel_variants"] = {}
+        for kern in ("pipe", "blocked", "lstage"):
+            for prec in (32, 64):
+                wv = Workload(args.config, prec, args.recon, dev, keep_host=False, kernel=kern)
+                rv = kernel_leg(timer, wv, half, args.warmup, world, peak)
+                line["kernel_variants"][f"{kern}_fp{prec}"] = {"us_per_launch": rv["us_per_launch"], "first_us": rv["first"]["us_per_launch"],
+                                                                "frac": rv["frac"], "sm_mhz": rv["clocks"]["sm_mhz"] if rv["clocks"] else None}
+                del wv
+                torch.cuda.empty_cache()
+        line["kernel_variants"]["note"] = ("same arithmetic, bit-identical results: pipe = persistent TMA pipeline (links + neighbour tiles staged), "
+                                           "blocked = gather kernel on 4-D boxes of warp tiles, lstage = gather kernel with TMA-staged links; "
+                                           "the primary line is the gather kernel")
     if want("recon18"):
         for prec in (32, 64):
             wv = Workload(args.config, prec, 18, dev, keep_host=False, kernel=args.kernel)

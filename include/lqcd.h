@@ -226,8 +226,9 @@ lqcd_status lqcd_cg_solve_tm_mixed(const lqcd_ctx* ctx64, const lqcd_ctx* ctx32,
 /* End-to-end path for host-resident data: canonical host buffers in, canonical host buffers out.
  * For each of the n items: copy in_host[i] (canonical half spinor of parity 1 - out_parity[i]) to the device,
  * pack, lqcd_dslash_eo, unpack, copy the canonical half spinor of parity out_parity[i] to out_host[i].
- * Items are pipelined over three device slots and three streams (upload / kernels on `stream` / download), so
- * both PCIe directions and the kernels overlap.  gauge_host: canonical links, uploaded and packed first; NULL
+ * Items are pipelined over three device slots and three streams (upload / kernels on `stream` / download; the two
+ * copy streams and the events are created at a context's first host-path call and released by lqcd_destroy), so
+ * both PCIe directions and the kernels overlap.  Host-path calls on one context are serialised.  gauge_host: canonical links, uploaded and packed first; NULL
  * reuses the links packed into workspace_dev by an earlier call.  workspace_dev: device scratch of
  * lqcd_host_workspace_bytes bytes, 256-byte aligned, owned by the caller.  Host buffers should be pinned
  * (pageable memory works, without overlap).  Work already enqueued on `stream` is ordered before the call; the
@@ -268,6 +269,8 @@ lqcd_status lqcd_plaquette(const lqcd_ctx* ctx, const void* links_canonical_dev,
 #define LQCD_KERNEL_GATHER 0
 #define LQCD_KERNEL_PIPE 1
 #define LQCD_KERNEL_BLOCKED 2 /* the gather kernel with the blocked thread -> site map (4-D boxes of warp tiles per block) */
+#define LQCD_KERNEL_LSTAGE 3  /* the gather kernel with the link stream staged through shared memory by the TMA unit
+                                 (every warp double-buffers its tile's link blocks with cp.async.bulk); precision 32 / 64 */
 lqcd_status lqcd_set_kernel(lqcd_ctx* ctx, int kernel);
 
 /* Number of kernels this library has launched since load (a claim counter for bench.py). */

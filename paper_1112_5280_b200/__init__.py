@@ -14,7 +14,7 @@ from . import _build
 
 LQCD_OK, LQCD_EINVAL, LQCD_EALIGN, LQCD_EALIAS, LQCD_EUNSUPPORTED, LQCD_ECUDA = range(6)
 PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, -1
-KERNEL_GATHER, KERNEL_PIPE, KERNEL_BLOCKED = 0, 1, 2
+KERNEL_GATHER, KERNEL_PIPE, KERNEL_BLOCKED, KERNEL_LSTAGE = 0, 1, 2, 3
 HAS_RECON8 = True
 
 EXPORTS = [

@@ -55,15 +55,48 @@ __device__ __forceinline__ void unpack(const double4_& w, double* v) {
     for (int i = 0; i < 4; ++i) v[i] = w.v[i];
 }
 
+// cache-policy experiments: spinor gathers 0 = default, 1 = L2::evict_last; 256-bit link words 0 =
+// default read-only path, 1 = .cs (evict-first), 2 = nc.L1::no_allocate.L2::evict_first; stores 0 = default, 1 = .cs
+#ifndef LQCD_SPINOR_POLICY
+#define LQCD_SPINOR_POLICY 0
+#endif
+#ifndef LQCD_LINK256_POLICY
+#define LQCD_LINK256_POLICY 0
+#endif
+#ifndef LQCD_STORE_POLICY
+#define LQCD_STORE_POLICY 0
+#endif
+#if LQCD_SPINOR_POLICY == 1
+#define LQCD_LD_SPINOR "ld.global.nc.L2::evict_last"
+#else
+#define LQCD_LD_SPINOR "ld.global.nc"
+#endif
+#if LQCD_STORE_POLICY == 1
+#define LQCD_ST_SPINOR "st.global.cs"
+#else
+#define LQCD_ST_SPINOR "st.global"
+#endif
 __device__ __forceinline__ float8_ ldg256(const float8_* p) {
     float8_ w;
-    asm("ld.global.nc.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+    asm(LQCD_LD_SPINOR ".v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
         : "=f"(w.v[0]), "=f"(w.v[1]), "=f"(w.v[2]), "=f"(w.v[3]), "=f"(w.v[4]), "=f"(w.v[5]), "=f"(w.v[6]), "=f"(w.v[7]) : "l"(p));
     return w;
 }
 __device__ __forceinline__ double4_ ldg256(const double4_* p) {
     double4_ w;
+    asm(LQCD_LD_SPINOR ".v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(w.v[0]), "=d"(w.v[1]), "=d"(w.v[2]), "=d"(w.v[3]) : "l"(p));
+    return w;
+}
+// 256-bit link words (fp64 12-real / 8-real storage): read exactly once per application
+__device__ __forceinline__ double4_ ldg256_stream(const double4_* p) {
+    double4_ w;
+#if LQCD_LINK256_POLICY == 1
+    asm("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(w.v[0]), "=d"(w.v[1]), "=d"(w.v[2]), "=d"(w.v[3]) : "l"(p));
+#elif LQCD_LINK256_POLICY == 2
+    asm("ld.global.nc.L1::no_allocate.L2::evict_first.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(w.v[0]), "=d"(w.v[1]), "=d"(w.v[2]), "=d"(w.v[3]) : "l"(p));
+#else
     asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(w.v[0]), "=d"(w.v[1]), "=d"(w.v[2]), "=d"(w.v[3]) : "l"(p));
+#endif
     return w;
 }
 // Plain (coherent) 256-bit loads for operands the same kernel overwrites (the in-place BLAS-1 updates): .nc is only
@@ -81,11 +114,11 @@ __device__ __forceinline__ double4_ ld256(const double4_* p) {
     return w;
 }
 __device__ __forceinline__ void stg256(float8_* p, const float* v) {
-    asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]),
+    asm volatile(LQCD_ST_SPINOR ".v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]),
                  "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
 }
 __device__ __forceinline__ void stg256(double4_* p, const double* v) {
-    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v[0]), "d"(v[1]), "d"(v[2]), "d"(v[3]) : "memory");
+    asm volatile(LQCD_ST_SPINOR ".v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v[0]), "d"(v[1]), "d"(v[2]), "d"(v[3]) : "memory");
 }
 
 // word 0 of site cb in a native half spinor; word q is q * TILE words further on
@@ -143,7 +176,7 @@ __device__ __forceinline__ void store_spinor(R* __restrict__ base, int cb, const
 __device__ __forceinline__ float4  ld_stream(const float4* p)  { return __ldcs(p); }
 __device__ __forceinline__ float2  ld_stream(const float2* p)  { return __ldcs(p); }
 __device__ __forceinline__ double2 ld_stream(const double2* p) { return __ldcs(p); }
-__device__ __forceinline__ double4_ ld_stream(const double4_* p) { return ldg256(p); }  // 256-bit: no .cs form; policy is immaterial here
+__device__ __forceinline__ double4_ ld_stream(const double4_* p) { return ldg256_stream(p); }
 
 // K2: rebuild row 2 of u[18] (row-major 3x3 complex, u[6 row + 2 col + reim]) as conj(row0 x row1);
 // valid for det U = +1 ("RECONSTRUCT TWELVE").

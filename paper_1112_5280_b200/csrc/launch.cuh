@@ -4,17 +4,30 @@
 #pragma once
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
 
 #include "../../include/lqcd.h"
 
 #include "dslash_kernel.cuh"
 #include "pipe_kernel.cuh"
+#include "lstage_kernel.cuh"
+
+// streams and events of the host-buffer path (lqcd_dslash_eo_host_batch), created at its first call and kept for
+// the life of the context; the mutex serialises host-path calls on one context (each call synchronises anyway)
+struct lqcd_host_pipe {
+    static constexpr int SLOTS = 3;
+    std::mutex lock;
+    bool ready = false;
+    cudaStream_t up = nullptr, down = nullptr;
+    cudaEvent_t start = nullptr, in_done[SLOTS] = {}, comp_done[SLOTS] = {}, out_done[SLOTS] = {};
+};
 
 struct lqcd_ctx {
     lqcd_params p;
     lqcd::Geom g;
     bool complex_bc;
-    int kernel;   // LQCD_KERNEL_GATHER or LQCD_KERNEL_PIPE (lqcd_set_kernel)
+    int kernel;   // LQCD_KERNEL_GATHER, _PIPE or _BLOCKED (lqcd_set_kernel)
+    mutable lqcd_host_pipe host;
 };
 
 namespace lqcd {
@@ -93,16 +106,31 @@ inline BlockMap box_shape(int nwarps, const Geom& g) {
     return m;
 }
 
+// gather kernel with the link stream staged by TMA (lstage_kernel.cuh); the range must start on a tile boundary
+template <typename R, int RECON, int EPI, bool CBC>
+lqcd_status launch_lstage(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
+                          const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
+    constexpr int BLOCK = DSLASH_BLOCK;
+    const int smem = LStage<R, RECON>::smem_bytes(BLOCK);
+    const dim3 grid((rg.end - rg.begin + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
+    const Epilogue<R> epi{(R)e.a, (R)e.g_re, (R)e.g_im, e.g5_out};
+    dslash_lstage_kernel<R, RECON, EPI, CBC, BLOCK><<<grid, BLOCK, smem, st>>>(
+        (R*)out, (const R*)gauge, (const R*)in, (const R*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<R>(c), rg.begin, rg.end);
+    return after_launch();
+}
+
 template <typename S, int RECON, int EPI, bool CBC>
 lqcd_status launch_one(const lqcd_ctx* c, void* out, const void* gauge, const void* in, const void* xin,
                        const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
     if constexpr (pipe_capable<S, RECON>) {
         if (c->kernel == LQCD_KERNEL_PIPE) return launch_pipe<S, RECON, EPI, CBC>(c, out, gauge, in, xin, e, parity, st, rg);
+        if (c->kernel == LQCD_KERNEL_LSTAGE && rg.begin % TILE == 0) return launch_lstage<S, RECON, EPI, CBC>(c, out, gauge, in, xin, e, parity, st, rg);
     }
     using A = typename Compute<S>::type;  // S is the storage type, A the arithmetic type
     const Epilogue<A> epi{(A)e.a, (A)e.g_re, (A)e.g_im, e.g5_out};
     // blocked map: all warps the register budget allows per SM in ONE block, on a compact box of warp tiles
     constexpr int NWARPS = MinBlocks<S, RECON>::value * 2;
+    if constexpr (EPI == EPI_STORE)   // an experiment: only the plain dslash is instantiated with the blocked map
     if (c->kernel == LQCD_KERNEL_BLOCKED && rg.begin == 0 && rg.end == c->g.Vh && c->g.sz % TILE == 0) {
         BlockMap m = box_shape(NWARPS, c->g);
         const dim3 grid(m.gy * m.gz * ((c->g.T + m.bt - 1) / m.bt), parity < 0 ? 2 : 1);
@@ -112,6 +140,16 @@ lqcd_status launch_one(const lqcd_ctx* c, void* out, const void* gauge, const vo
     }
     constexpr int BLOCK = DSLASH_BLOCK;
     const dim3 grid((rg.end - rg.begin + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
+#ifdef LQCD_CARVEOUT_EXPERIMENT   // how much L1 the gather kernel needs: $LQCD_CARVEOUT = per cent of the 228 KB given to shared memory
+    {
+        static int done = 0;
+        if (!done) {
+            if (const char* e = std::getenv("LQCD_CARVEOUT"))
+                cudaFuncSetAttribute(dslash_kernel<S, RECON, EPI, CBC, BLOCK>, cudaFuncAttributePreferredSharedMemoryCarveout, std::atoi(e));
+            done = 1;
+        }
+    }
+#endif
     dslash_kernel<S, RECON, EPI, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
         (S*)out, (const S*)gauge, (const S*)in, (const S*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<A>(c), rg.begin, rg.end, BlockMap{0, 0, 0, 0, 0, 0});
     return after_launch();

@@ -69,7 +69,7 @@ inline size_t half_bytes(const lqcd_ctx* c) {
     return (size_t)TILE * c->g.ntiles * (24 * elem(c) + (c->p.precision == 16 ? 4 : 0));
 }
 inline size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
-constexpr int HOST_SLOTS = 3;  // pipeline depth of lqcd_dslash_eo_host_batch
+constexpr int HOST_SLOTS = lqcd_host_pipe::SLOTS;  // pipeline depth of lqcd_dslash_eo_host_batch
 
 inline CbRange all_sites(const lqcd_ctx* c) { return CbRange{0, c->g.Vh}; }
 
@@ -138,6 +138,17 @@ lqcd_status lqcd_create(lqcd_ctx** ctx, const lqcd_params* p) {
 }
 
 lqcd_status lqcd_destroy(lqcd_ctx* ctx) {
+    if (ctx && ctx->host.ready) {
+        lqcd_host_pipe& h = ctx->host;
+        for (int k = 0; k < lqcd_host_pipe::SLOTS; ++k) {
+            cudaEventDestroy(h.in_done[k]);
+            cudaEventDestroy(h.comp_done[k]);
+            cudaEventDestroy(h.out_done[k]);
+        }
+        cudaEventDestroy(h.start);
+        cudaStreamDestroy(h.up);
+        cudaStreamDestroy(h.down);
+    }
     delete ctx;
     return LQCD_OK;
 }
@@ -237,8 +248,8 @@ lqcd_status lqcd_unpack_spinor(const lqcd_ctx* c, void* canon, const void* nativ
 }
 
 lqcd_status lqcd_set_kernel(lqcd_ctx* c, int kernel) {
-    if (!c || (kernel != LQCD_KERNEL_GATHER && kernel != LQCD_KERNEL_PIPE && kernel != LQCD_KERNEL_BLOCKED)) return LQCD_EINVAL;
-    if (kernel == LQCD_KERNEL_PIPE && (c->p.precision == 16 || c->p.link_precision == 16)) return LQCD_EUNSUPPORTED;
+    if (!c || kernel < LQCD_KERNEL_GATHER || kernel > LQCD_KERNEL_LSTAGE) return LQCD_EINVAL;
+    if ((kernel == LQCD_KERNEL_PIPE || kernel == LQCD_KERNEL_LSTAGE) && (c->p.precision == 16 || c->p.link_precision == 16)) return LQCD_EUNSUPPORTED;
     c->kernel = kernel;
     return LQCD_OK;
 }
@@ -627,19 +638,26 @@ lqcd_status lqcd_dslash_eo_host_batch(const lqcd_ctx* c, int n, void* const* out
     }
     cudaError_t e = cudaSuccess;
     lqcd_status s = LQCD_OK;
-    cudaStream_t up = nullptr, down = nullptr;
-    cudaEvent_t start = nullptr, in_done[HOST_SLOTS] = {}, comp_done[HOST_SLOTS] = {}, out_done[HOST_SLOTS] = {};
     auto fail = [&](cudaError_t err) { e = err; return err != cudaSuccess; };
-    do {
-        if (fail(cudaStreamCreateWithFlags(&up, cudaStreamNonBlocking))) break;
-        if (fail(cudaStreamCreateWithFlags(&down, cudaStreamNonBlocking))) break;
-        if (fail(cudaEventCreateWithFlags(&start, cudaEventDisableTiming))) break;
-        bool ok = true;
+    lqcd_host_pipe& hp = c->host;
+    std::lock_guard<std::mutex> guard(hp.lock);
+    if (!hp.ready) {   // first host-path call on this context: two copy streams and the events that order the slots
+        bool ok = !fail(cudaStreamCreateWithFlags(&hp.up, cudaStreamNonBlocking)) &&
+                  !fail(cudaStreamCreateWithFlags(&hp.down, cudaStreamNonBlocking)) &&
+                  !fail(cudaEventCreateWithFlags(&hp.start, cudaEventDisableTiming));
         for (int k = 0; k < HOST_SLOTS && ok; ++k)
-            ok = !fail(cudaEventCreateWithFlags(&in_done[k], cudaEventDisableTiming)) &&
-                 !fail(cudaEventCreateWithFlags(&comp_done[k], cudaEventDisableTiming)) &&
-                 !fail(cudaEventCreateWithFlags(&out_done[k], cudaEventDisableTiming));
-        if (!ok) break;
+            ok = !fail(cudaEventCreateWithFlags(&hp.in_done[k], cudaEventDisableTiming)) &&
+                 !fail(cudaEventCreateWithFlags(&hp.comp_done[k], cudaEventDisableTiming)) &&
+                 !fail(cudaEventCreateWithFlags(&hp.out_done[k], cudaEventDisableTiming));
+        if (!ok) return cuda_fail(e);   // a context whose host path could not be set up keeps failing here
+        hp.ready = true;
+    }
+    const cudaStream_t up = hp.up, down = hp.down;
+    const cudaEvent_t start = hp.start;
+    cudaEvent_t* const in_done = hp.in_done;
+    cudaEvent_t* const comp_done = hp.comp_done;
+    cudaEvent_t* const out_done = hp.out_done;
+    do {
         // everything already enqueued on the caller's stream comes first
         if (fail(cudaEventRecord(start, st)) || fail(cudaStreamWaitEvent(up, start, 0)) || fail(cudaStreamWaitEvent(down, start, 0))) break;
         if (gauge_host) {
@@ -665,19 +683,11 @@ lqcd_status lqcd_dslash_eo_host_batch(const lqcd_ctx* c, int n, void* const* out
             if (fail(cudaEventRecord(out_done[k], down))) break;
         }
     } while (false);
-    // drain all three streams before the events and streams go away (also on the error paths)
-    if (up) cudaStreamSynchronize(up);
-    if (down) cudaStreamSynchronize(down);
+    // drain all three streams before returning (also on the error paths): the results live in host memory
+    cudaStreamSynchronize(up);
+    cudaStreamSynchronize(down);
     const cudaError_t es = cudaStreamSynchronize(st);
     if (e == cudaSuccess) e = es;
-    for (int k = 0; k < HOST_SLOTS; ++k) {
-        if (in_done[k]) cudaEventDestroy(in_done[k]);
-        if (comp_done[k]) cudaEventDestroy(comp_done[k]);
-        if (out_done[k]) cudaEventDestroy(out_done[k]);
-    }
-    if (start) cudaEventDestroy(start);
-    if (up) cudaStreamDestroy(up);
-    if (down) cudaStreamDestroy(down);
     if (s != LQCD_OK) return s;
     return e == cudaSuccess ? LQCD_OK : cuda_fail(e);
 }

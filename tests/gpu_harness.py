@@ -41,7 +41,7 @@ class Gpu:
         if kernel is None and precision != 16 and not link_precision:
             kernel = os.environ.get("LQCD_TEST_KERNEL")
         if kernel is not None:
-            self.ctx.set_kernel({"gather": L.KERNEL_GATHER, "pipe": L.KERNEL_PIPE, "blocked": L.KERNEL_BLOCKED}[kernel])
+            self.ctx.set_kernel({"gather": L.KERNEL_GATHER, "pipe": L.KERNEL_PIPE, "blocked": L.KERNEL_BLOCKED, "lstage": L.KERNEL_LSTAGE}[kernel])
         self.dims, self.precision = tuple(dims), precision
         self.cd = cdtype(precision)
         self.dev = torch.device("cuda:0")

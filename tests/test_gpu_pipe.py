@@ -38,12 +38,13 @@ def _bc(bc):
 @pytest.mark.parametrize("precision", [64, 32])
 @pytest.mark.parametrize("recon", [18, 12, 8])
 @pytest.mark.parametrize("dims,bc", LATTICES)
-def test_pipe_eo_full_and_matrix(H, dims, bc, precision, recon):
+@pytest.mark.parametrize("kernel", ["pipe", "lstage"])
+def test_pipe_eo_full_and_matrix(H, dims, bc, precision, recon, kernel):
     bc = _bc(bc)
     cd = H.cdtype(precision)
     U = li.random_su3_links(dims, seed=31).astype(cd)
     psi = li.gaussian_spinor(dims, seed=32).astype(cd)
-    g = H.Gpu(dims, precision, recon, bc, U, kernel="pipe")
+    g = H.Gpu(dims, precision, recon, bc, U, kernel=kernel)
     ref_g = H.Gpu(dims, precision, recon, bc, U, kernel="gather")
     st = H.site_tol_for(U, precision, recon)
     for op in (0, 1):
@@ -64,7 +65,8 @@ def test_pipe_eo_full_and_matrix(H, dims, bc, precision, recon):
 
 
 @pytest.mark.parametrize("precision,recon", [(64, 12), (32, 12), (32, 18), (64, 8)])
-def test_pipe_many_tiles_per_cta(H, precision, recon):
+@pytest.mark.parametrize("kernel", ["pipe", "lstage"])
+def test_pipe_many_tiles_per_cta(H, precision, recon, kernel):
     """Config 3 (16^3x32: 2048 tiles per parity, ~14 per CTA): every ring slot is reused several times, by different
     consumer warps in turn."""
     c = li.CONFIGS[3]
@@ -72,7 +74,7 @@ def test_pipe_many_tiles_per_cta(H, precision, recon):
     cd = H.cdtype(precision)
     U = li.links_for_config(3).astype(cd)
     psi = li.gaussian_spinor(dims).astype(cd)
-    g = H.Gpu(dims, precision, recon, bc, U, kernel="pipe")
+    g = H.Gpu(dims, precision, recon, bc, U, kernel=kernel)
     ref_g = H.Gpu(dims, precision, recon, bc, U, kernel="gather")
     st = H.site_tol_for(U, precision, recon)
     for op in (0, 1):
@@ -84,14 +86,15 @@ def test_pipe_many_tiles_per_cta(H, precision, recon):
 
 
 @pytest.mark.parametrize("precision", [64, 32])
-def test_pipe_time_slice_ranges(H, precision):
+@pytest.mark.parametrize("kernel", ["pipe", "lstage"])
+def test_pipe_time_slice_ranges(H, precision, kernel):
     """lqcd_dslash_eo_range on the pipelined kernel: ranges that start and end inside tiles (z planes of 12 sites)."""
     import torch
     dims, bc = (4, 6, 4, 8), (1, 1, 1, -1)
     cd = H.cdtype(precision)
     U = li.random_su3_links(dims, seed=41).astype(cd)
     psi = li.gaussian_spinor(dims, seed=42).astype(cd)
-    g = H.Gpu(dims, precision, 12, bc, U, kernel="pipe")
+    g = H.Gpu(dims, precision, 12, bc, U, kernel=kernel)
     ref = H.half_of(oracle.dslash_eo(U, psi, dims, bc, 0), dims, 0)
     inp = g.to_native(H.half_of(psi, dims, 1), 1)
     out = g.buf()
