@@ -570,7 +570,7 @@ def cg_mixed_leg(torch, w64, w32, mu=0.05, tol=1e-10, inner_tol=1e-4, maxiter=20
 
 def heatbath_leg(torch, dev, cfg_id=4, beta=6.0, ntries=4, sweeps=3):
     """Next row f4, last clause: pure-gauge SU(3) heatbath sweeps (8 sublattice launches each) on the config's lattice,
-    fp64, canonical link field, uniforms drawn on the device beforehand (they are inputs of the method).  Bytes per link
+    fp64, link field in the update layout, uniforms drawn on the device beforehand (they are inputs of the method).  Bytes per link
     update (model): the 18 staple links and the link itself are shared with other updates -- each launch touches all
     links of the three other directions (3 V), the mu links of both parities (V) and writes V/2: 9 links of 144 B per
     update -- plus the uniforms of one attempt and the direction per subgroup (3 x 6 x 8 B)."""
@@ -579,7 +579,11 @@ def heatbath_leg(torch, dev, cfg_id=4, beta=6.0, ntries=4, sweeps=3):
     import paper_1112_5280_b200 as L
     c = li.CONFIGS[cfg_id]
     ctx = L.Context(c["dims"], 64, 18, (1, 1, 1, 1))
-    U = torch.from_numpy(li.links_for_config(cfg_id, dtype=np.complex128)).to(dev)
+    Uc = torch.from_numpy(li.links_for_config(cfg_id, dtype=np.complex128)).to(dev)
+    U = torch.empty(ctx.update_links_bytes(), dtype=torch.uint8, device=dev)   # the update layout (structure of arrays, checkerboarded)
+    ctx.pack_update_links(U, Uc)
+    torch.cuda.synchronize()
+    del Uc
     ws = torch.empty(ctx.plaquette_workspace_bytes(), dtype=torch.uint8, device=dev)
     p0 = ctx.plaquette(U, ws)
     n = ctx.heatbath_uniforms(ntries)

@@ -241,21 +241,27 @@ lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* ctx, void* out_host, const void*
 
 /* ---- pure-gauge SU(3) heatbath (next row f4; "On the PGT side we need a SU(3) heatbath algorithm [20]",
  * ref. [20] at :156: Creutz, Cabibbo-Marinari, Kennedy-Pendleton; reading F7) ----
- * Wilson action S = beta sum_p (1 - 1/3 Re tr U_p).  lqcd_heatbath_sublattice updates, in place, the links U_mu(x) of
- * one direction mu on the sites of one parity of a CANONICAL link field [mu 4][T][Z][Y][X][3][3] complex128 on the
- * device (precision-64 contexts only; links are periodic and carry no boundary phase): staple sum, then the SU(2)
- * subgroups (0,1), (0,2), (1,2), each drawn with the Kennedy-Pendleton sampler.  The uniform random numbers are an
- * INPUT: uniforms_dev holds lqcd_heatbath_uniforms(ctx, ntries) doubles in (0, 1], [site cb of the parity][subgroup 3]
- * [4 ntries + 2] (the 4 numbers of attempt t at [4 t, 4 t + 4), then cos(theta) and phi of the direction); a subgroup
- * with none of its ntries (1..64) attempts accepted is left unchanged.  Eight calls (mu = 0..3, parity 0, 1) are a
- * sweep; repack with lqcd_pack_gauge before the next dslash.  One launch, asynchronous on `stream`.
- * lqcd_plaquette: the average of 1/3 Re tr U_p over all 6 V plaquettes, to host (synchronises `stream`);
- * workspace_dev: lqcd_plaquette_workspace_bytes bytes, 256-byte aligned.  Deterministic reduction. */
+ * Wilson action S = beta sum_p (1 - 1/3 Re tr U_p).  The update kernels work on the UPDATE LAYOUT of the link field
+ * (precision-64 contexts only; links are periodic and carry no boundary phase): structure of arrays, checkerboarded --
+ * the complex128 word w = 3 row + col of U_mu(x), x of parity p and checkerboard index cb, at
+ * ((mu 2 + p) 9 + w) 32 ntiles + cb -- lqcd_update_links_bytes bytes, 16-byte aligned; lqcd_pack_update_links /
+ * lqcd_unpack_update_links convert from / to the canonical field [mu 4][T][Z][Y][X][3][3] complex128 on the device.
+ * lqcd_heatbath_sublattice updates, in place, the links U_mu(x) of one direction mu on the sites of one parity: staple
+ * sum, then the SU(2) subgroups (0,1), (0,2), (1,2), each drawn with the Kennedy-Pendleton sampler.  The uniform random
+ * numbers are an INPUT: uniforms_dev holds lqcd_heatbath_uniforms(ctx, ntries) doubles in (0, 1], [site cb of the parity]
+ * [subgroup 3][4 ntries + 2] (the 4 numbers of attempt t at [4 t, 4 t + 4), then cos(theta) and phi of the direction); a
+ * subgroup with none of its ntries (1..64) attempts accepted is left unchanged.  Eight calls (mu = 0..3, parity 0, 1) are
+ * a sweep; unpack and lqcd_pack_gauge before the next dslash.  One launch each, asynchronous on `stream`.
+ * lqcd_plaquette: the average of 1/3 Re tr U_p over all 6 V plaquettes of a field in the update layout, to host
+ * (synchronises `stream`); workspace_dev: lqcd_plaquette_workspace_bytes bytes, 256-byte aligned.  Deterministic. */
+size_t lqcd_update_links_bytes(const lqcd_ctx* ctx);
+lqcd_status lqcd_pack_update_links(const lqcd_ctx* ctx, void* update_dev, const void* canonical_dev, void* stream);
+lqcd_status lqcd_unpack_update_links(const lqcd_ctx* ctx, void* canonical_dev, const void* update_dev, void* stream);
 size_t lqcd_heatbath_uniforms(const lqcd_ctx* ctx, int ntries);
-lqcd_status lqcd_heatbath_sublattice(const lqcd_ctx* ctx, void* links_canonical_dev, double beta, int mu, int parity,
+lqcd_status lqcd_heatbath_sublattice(const lqcd_ctx* ctx, void* links_update_dev, double beta, int mu, int parity,
                                      const void* uniforms_dev, int ntries, void* stream);
 size_t lqcd_plaquette_workspace_bytes(const lqcd_ctx* ctx);
-lqcd_status lqcd_plaquette(const lqcd_ctx* ctx, const void* links_canonical_dev, void* workspace_dev, double* plaq_host,
+lqcd_status lqcd_plaquette(const lqcd_ctx* ctx, const void* links_update_dev, void* workspace_dev, double* plaq_host,
                            void* stream);
 
 /* Which kernel the hot-path entry points of this ctx launch (same arithmetic, same results up to the order of the

@@ -9,11 +9,17 @@
 // the action); one thread per link: six staples (12 products of 3x3 matrices, 18 gathered links), then the three
 // Cabibbo-Marinari subgroup steps (0,1), (0,2), (1,2), each drawing its SU(2) element with the Kennedy-Pendleton
 // sampler from uniforms the CALLER supplies (uniforms[cb][subgroup][4 ntries + 2]; at most ntries attempts, a subgroup
-// with no accepted attempt is left alone).  Works on the canonical link field [mu][T][Z][Y][X][3][3] complex128 in
-// place: a link is 144 contiguous bytes, so even the every-other-site access of a checkerboard wastes only the sectors
-// at the seams, and the repack for the dslash kernels (lqcd_pack_gauge) is needed once per configuration anyway.
-// fp64 only.  Links are periodic and carry no boundary phase.
+// with no accepted attempt is left alone).
+//
+// Layout: the "update layout" of the link field, structure of arrays and checkerboarded like the spinors of the dslash:
+//   double2 word w = 3 row + col of U_mu(x), x of parity p and checkerboard index cb, at
+//   ((mu 2 + p) 9 + w) Vp + cb,   Vp = 32 ntiles (sites per parity, padded to whole tiles)
+// so the 32 lanes of a warp read one word of 32 consecutive sites as one 512-byte run, for the thread's own link and
+// (up to lattice wrap-arounds) for each of the 18 staple links.  lqcd_pack_update_links / lqcd_unpack_update_links
+// convert from / to the canonical [mu][T][Z][Y][X][3][3] complex128 field.  fp64 only.  Links are periodic and carry no
+// boundary phase.
 #pragma once
+#include "fields.cuh"
 #include "geometry.cuh"
 
 namespace lqcd {
@@ -26,13 +32,18 @@ constexpr int HB_BLOCK = 128;
 
 struct Mat3 { double re[9], im[9]; };   // row-major: element (r, c) at 3 r + c
 
+// word 0 of U_mu(x) for x = (parity p, checkerboard index cb); word w is w Vp further on
+__host__ __device__ __forceinline__ size_t update_word0(int ntiles, int mu, int p, int cb) {
+    return (size_t)((mu * 2 + p) * 9) * ((size_t)TILE * ntiles) + cb;
+}
 // RO: the link is not written by the running launch (every link but the thread's own): read-only path
 template <bool RO = true>
-__device__ __forceinline__ void load_mat(const double* links, size_t link, Mat3& m) {
-    const double2* p = reinterpret_cast<const double2*>(links) + link * 9;
+__device__ __forceinline__ void load_mat(const double2* links, int ntiles, int mu, int p, int cb, Mat3& m) {
+    const double2* q = links + update_word0(ntiles, mu, p, cb);
+    const size_t Vp = (size_t)TILE * ntiles;
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
-        const double2 z = RO ? __ldg(p + k) : p[k];
+        const double2 z = RO ? __ldg(q + k * Vp) : q[k * Vp];
         m.re[k] = z.x;
         m.im[k] = z.y;
     }
@@ -57,22 +68,6 @@ __device__ __forceinline__ void mul(const Mat3& a, const Mat3& b, Mat3& c) {
             c.re[3 * r + s] = xr;
             c.im[3 * r + s] = xi;
         }
-}
-
-// coordinates of a site and its lexicographic index; run-time directions are resolved with selects, not indexed arrays
-// (which would live in local memory)
-struct Coords { int c0, c1, c2, c3; size_t lex; };
-__device__ __forceinline__ int coord(const Coords& c, int mu) { return mu == 0 ? c.c0 : (mu == 1 ? c.c1 : (mu == 2 ? c.c2 : c.c3)); }
-__device__ __forceinline__ int extent(const Geom& g, int mu) { return mu == 0 ? g.X : (mu == 1 ? g.Y : (mu == 2 ? g.Z : g.T)); }
-__device__ __forceinline__ long long stride(const Geom& g, int mu) {
-    return mu == 0 ? 1 : (mu == 1 ? g.X : (mu == 2 ? (long long)g.X * g.Y : (long long)g.X * g.Y * g.Z));
-}
-// lexicographic index of the site one step (d = +1 / -1) along mu from c, periodic
-__device__ __forceinline__ size_t hop(const Geom& g, const Coords& c, size_t lex, int mu, int d) {
-    const int x = coord(c, mu), L = extent(g, mu);
-    const long long st = stride(g, mu);
-    if (d > 0) return x == L - 1 ? lex - (size_t)((L - 1) * st) : lex + (size_t)st;
-    return x == 0 ? lex + (size_t)((L - 1) * st) : lex - (size_t)st;
 }
 
 // One Cabibbo-Marinari step in the block (I, J) on the link u with staple sum a: u <- G u.
@@ -135,22 +130,15 @@ __device__ __forceinline__ void subgroup_step(Mat3& u, const Mat3& a, double bet
     }
 }
 
-__device__ __forceinline__ Coords site_coords(const Geom& g, int cb, int parity) {
-    const Site s = decode_site(g, cb, parity);
-    Coords c;
-    c.c0 = 2 * s.xh + s.x_odd; c.c1 = s.y; c.c2 = s.z; c.c3 = s.t;
-    c.lex = (size_t)2 * cb + s.x_odd;
-    return c;
-}
-
-// links: canonical [mu][V][3][3] complex128, updated in place for (mu, parity); uniforms: [V/2][3][4 ntries + 2]
-__global__ void __launch_bounds__(HB_BLOCK, LQCD_HB_MINB) heatbath_kernel(double* links, Geom g, double beta, int mu, int parity,
-                                                            const double* __restrict__ uniforms, int ntries) {
+// links: update layout, updated in place for (mu, parity); uniforms: [V/2][3][4 ntries + 2]
+__global__ void __launch_bounds__(HB_BLOCK, LQCD_HB_MINB) heatbath_kernel(double2* links, Geom g, double beta, int mu, int parity,
+                                                                          const double* __restrict__ uniforms, int ntries) {
     const int cb = blockIdx.x * HB_BLOCK + threadIdx.x;
     if (cb >= g.Vh) return;
-    const Coords c = site_coords(g, cb, parity);
-    const size_t V = (size_t)2 * g.Vh;
-    const size_t x0 = c.lex, xmu = hop(g, c, x0, mu, +1);
+    const int p = parity, q = 1 - parity, nt = g.ntiles;
+    const Site s = decode_site(g, cb, p);
+    const int xmu = neighbour_rt(g, cb, s, 2 * mu);               // x + mu^, a site of parity q
+    const Site smu = decode_site(g, xmu, q);
     Mat3 a;
 #pragma unroll
     for (int k = 0; k < 9; ++k) a.re[k] = a.im[k] = 0.0;
@@ -158,71 +146,82 @@ __global__ void __launch_bounds__(HB_BLOCK, LQCD_HB_MINB) heatbath_kernel(double
     // nothing this launch writes
     for (int nu = 0; nu < 4; ++nu) {
         if (nu == mu) continue;
-        Mat3 p, q, t;
+        Mat3 m1, m2, t;
         // upper staple  U_nu(x+mu) U_mu(x+nu)^+ U_nu(x)^+
-        load_mat(links, nu * V + xmu, p);
-        load_mat(links, mu * V + hop(g, c, x0, nu, +1), q);
-        mul<false, true>(p, q, t);
-        load_mat(links, nu * V + x0, p);
-        mul<false, true>(t, p, q);
+        load_mat(links, nt, nu, q, xmu, m1);
+        load_mat(links, nt, mu, q, neighbour_rt(g, cb, s, 2 * nu), m2);
+        mul<false, true>(m1, m2, t);
+        load_mat(links, nt, nu, p, cb, m1);
+        mul<false, true>(t, m1, m2);
 #pragma unroll
-        for (int k = 0; k < 9; ++k) { a.re[k] += q.re[k]; a.im[k] += q.im[k]; }
+        for (int k = 0; k < 9; ++k) { a.re[k] += m2.re[k]; a.im[k] += m2.im[k]; }
         // lower staple  U_nu(x+mu-nu)^+ U_mu(x-nu)^+ U_nu(x-nu)
-        const size_t xdn = hop(g, c, x0, nu, -1);
-        load_mat(links, nu * V + hop(g, c, xmu, nu, -1), p);   // x + mu^ - nu^: the nu coordinate of x + mu^ is that of x
-        load_mat(links, mu * V + xdn, q);
-        mul<true, true>(p, q, t);
-        load_mat(links, nu * V + xdn, p);
-        mul<false, false>(t, p, q);
+        const int xdn = neighbour_rt(g, cb, s, 2 * nu + 1);       // x - nu^, parity q
+        load_mat(links, nt, nu, p, neighbour_rt(g, xmu, smu, 2 * nu + 1), m1);   // x + mu^ - nu^, parity p
+        load_mat(links, nt, mu, q, xdn, m2);
+        mul<true, true>(m1, m2, t);
+        load_mat(links, nt, nu, q, xdn, m1);
+        mul<false, false>(t, m1, m2);
 #pragma unroll
-        for (int k = 0; k < 9; ++k) { a.re[k] += q.re[k]; a.im[k] += q.im[k]; }
+        for (int k = 0; k < 9; ++k) { a.re[k] += m2.re[k]; a.im[k] += m2.im[k]; }
     }
     Mat3 u;
-    load_mat<false>(links, mu * V + x0, u);
+    load_mat<false>(links, nt, mu, p, cb, u);
     const double* r = uniforms + (size_t)cb * 3 * (4 * ntries + 2);
     subgroup_step<0, 1>(u, a, beta, r, ntries);
     subgroup_step<0, 2>(u, a, beta, r + (4 * ntries + 2), ntries);
     subgroup_step<1, 2>(u, a, beta, r + 2 * (4 * ntries + 2), ntries);
-    double2* out = reinterpret_cast<double2*>(links) + (mu * V + x0) * 9;
+    double2* out = links + update_word0(nt, mu, p, cb);
+    const size_t Vp = (size_t)TILE * nt;
 #pragma unroll
-    for (int k = 0; k < 9; ++k) out[k] = make_double2(u.re[k], u.im[k]);
+    for (int k = 0; k < 9; ++k) out[k * Vp] = make_double2(u.re[k], u.im[k]);
 }
 
-// partial[block] = sum over the block's sites (both parities: thread = lexicographic site) of the 6 Re tr U_p
-__global__ void __launch_bounds__(HB_BLOCK) plaquette_kernel(const double* __restrict__ links, Geom g, double* __restrict__ partial) {
-    const size_t V = (size_t)2 * g.Vh;
-    const size_t lex = (size_t)blockIdx.x * HB_BLOCK + threadIdx.x;
-    double s = 0.0;
-    if (lex < V) {
-        Coords c;
-        size_t r = lex;
-        c.c0 = (int)(r % g.X); r /= g.X;
-        c.c1 = (int)(r % g.Y); r /= g.Y;
-        c.c2 = (int)(r % g.Z); c.c3 = (int)(r / g.Z);
-        c.lex = lex;
+// partial[blockIdx.y gridDim.x + blockIdx.x] = sum over the block's sites of parity blockIdx.y of the 6 Re tr U_p
+__global__ void __launch_bounds__(HB_BLOCK) plaquette_kernel(const double2* __restrict__ links, Geom g, double* __restrict__ partial) {
+    const int cb = blockIdx.x * HB_BLOCK + threadIdx.x, p = blockIdx.y, q = 1 - p, nt = g.ntiles;
+    double sum = 0.0;
+    if (cb < g.Vh) {
+        const Site s = decode_site(g, cb, p);
         for (int mu = 0; mu < 4; ++mu)
             for (int nu = mu + 1; nu < 4; ++nu) {
-                Mat3 p, q, t;
-                load_mat(links, mu * V + lex, p);
-                load_mat(links, nu * V + hop(g, c, lex, mu, +1), q);
-                mul<false, false>(p, q, t);
-                load_mat(links, mu * V + hop(g, c, lex, nu, +1), p);
-                mul<false, true>(t, p, q);
-                load_mat(links, nu * V + lex, p);
-                // Re tr(q p^+) = sum_rc Re(q_rc conj(p_rc))
+                Mat3 m1, m2, t;
+                load_mat(links, nt, mu, p, cb, m1);
+                load_mat(links, nt, nu, q, neighbour_rt(g, cb, s, 2 * mu), m2);
+                mul<false, false>(m1, m2, t);
+                load_mat(links, nt, mu, q, neighbour_rt(g, cb, s, 2 * nu), m1);
+                mul<false, true>(t, m1, m2);
+                load_mat(links, nt, nu, p, cb, m1);
+                // Re tr(m2 m1^+) = sum_rc Re(m2_rc conj(m1_rc))
 #pragma unroll
-                for (int k = 0; k < 9; ++k) s += q.re[k] * p.re[k] + q.im[k] * p.im[k];
+                for (int k = 0; k < 9; ++k) sum += m2.re[k] * m1.re[k] + m2.im[k] * m1.im[k];
             }
     }
     __shared__ double warp_sums[HB_BLOCK / 32];
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
-    if ((threadIdx.x & 31) == 0) warp_sums[threadIdx.x >> 5] = s;
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
+    if ((threadIdx.x & 31) == 0) warp_sums[threadIdx.x >> 5] = sum;
     __syncthreads();
     if (threadIdx.x == 0) {
         double tot = 0.0;
         for (int w = 0; w < HB_BLOCK / 32; ++w) tot += warp_sums[w];
-        partial[blockIdx.x] = tot;
+        partial[blockIdx.y * gridDim.x + blockIdx.x] = tot;
+    }
+}
+
+// canonical [mu][V][3][3] complex128 <-> update layout; grid (ceil(Vh / block), 4 directions, 2 parities)
+template <bool UNPACK>
+__global__ void __launch_bounds__(HB_BLOCK) update_links_pack_kernel(double2* native, double2* canon, Geom g) {
+    const int cb = blockIdx.x * HB_BLOCK + threadIdx.x;
+    if (cb >= g.Vh) return;
+    const int mu = blockIdx.y, p = blockIdx.z;
+    const Site s = decode_site(g, cb, p);
+    const size_t lex = (size_t)2 * cb + s.x_odd, V = (size_t)2 * g.Vh, Vp = (size_t)TILE * g.ntiles;
+    double2* c = canon + (mu * V + lex) * 9;
+    double2* n = native + update_word0(g.ntiles, mu, p, cb);
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        if (UNPACK) c[k] = n[k * Vp]; else n[k * Vp] = c[k];
     }
 }
 

@@ -700,7 +700,27 @@ lqcd_status lqcd_dslash_eo_host(const lqcd_ctx* c, void* out_host, const void* g
     return lqcd_dslash_eo_host_batch(c, 1, outs, gauge_host, ins, &out_parity, ws, stream);
 }
 
-// ---- next row f4, last clause: pure-gauge heatbath on the canonical link field (heatbath_kernels.cuh) -------------------
+// ---- next row f4, last clause: pure-gauge heatbath on the update layout of the links (heatbath_kernels.cuh) -----------
+size_t lqcd_update_links_bytes(const lqcd_ctx* c) { return c ? (size_t)4 * 2 * 9 * TILE * c->g.ntiles * sizeof(double2) : 0; }
+
+static lqcd_status update_links_convert(const lqcd_ctx* c, void* native, void* canon, void* stream, bool unpack) {
+    if (!c || !native || !canon) return LQCD_EINVAL;
+    if (c->p.precision != 64) return LQCD_EUNSUPPORTED;   // complex128 links
+    if (!aligned16(native) || !aligned16(canon)) return LQCD_EALIGN;
+    const dim3 grid((c->g.Vh + HB_BLOCK - 1) / HB_BLOCK, 4, 2);
+    if (unpack) update_links_pack_kernel<true><<<grid, HB_BLOCK, 0, (cudaStream_t)stream>>>((double2*)native, (double2*)canon, c->g);
+    else update_links_pack_kernel<false><<<grid, HB_BLOCK, 0, (cudaStream_t)stream>>>((double2*)native, (double2*)canon, c->g);
+    return after_launch();
+}
+
+lqcd_status lqcd_pack_update_links(const lqcd_ctx* c, void* native, const void* canon, void* stream) {
+    return update_links_convert(c, native, const_cast<void*>(canon), stream, false);
+}
+
+lqcd_status lqcd_unpack_update_links(const lqcd_ctx* c, void* canon, const void* native, void* stream) {
+    return update_links_convert(c, const_cast<void*>(native), canon, stream, true);
+}
+
 size_t lqcd_heatbath_uniforms(const lqcd_ctx* c, int ntries) {
     return c && ntries > 0 ? (size_t)c->g.Vh * 3 * (4 * (size_t)ntries + 2) : 0;
 }
@@ -709,15 +729,15 @@ lqcd_status lqcd_heatbath_sublattice(const lqcd_ctx* c, void* links, double beta
                                      int ntries, void* stream) {
     if (!c || !links || !uniforms) return LQCD_EINVAL;
     if (mu < 0 || mu > 3 || (parity != 0 && parity != 1) || ntries < 1 || ntries > 64 || !(beta > 0.0)) return LQCD_EINVAL;
-    if (c->p.precision != 64) return LQCD_EUNSUPPORTED;   // the canonical field of a precision-64 context (complex128)
+    if (c->p.precision != 64) return LQCD_EUNSUPPORTED;
     if (!aligned16(links) || (reinterpret_cast<uintptr_t>(uniforms) & 7u)) return LQCD_EALIGN;
     heatbath_kernel<<<(c->g.Vh + HB_BLOCK - 1) / HB_BLOCK, HB_BLOCK, 0, (cudaStream_t)stream>>>(
-        (double*)links, c->g, beta, mu, parity, (const double*)uniforms, ntries);
+        (double2*)links, c->g, beta, mu, parity, (const double*)uniforms, ntries);
     return after_launch();
 }
 
 size_t lqcd_plaquette_workspace_bytes(const lqcd_ctx* c) {
-    return c ? align256((size_t)((2 * (size_t)c->g.Vh + HB_BLOCK - 1) / HB_BLOCK) * sizeof(double)) + 256 : 0;
+    return c ? align256((size_t)2 * ((c->g.Vh + HB_BLOCK - 1) / HB_BLOCK) * sizeof(double)) + 256 : 0;
 }
 
 lqcd_status lqcd_plaquette(const lqcd_ctx* c, const void* links, void* workspace, double* plaq_host, void* stream) {
@@ -725,20 +745,19 @@ lqcd_status lqcd_plaquette(const lqcd_ctx* c, const void* links, void* workspace
     if (c->p.precision != 64) return LQCD_EUNSUPPORTED;
     if (!aligned16(links) || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return LQCD_EALIGN;
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t V = 2 * (size_t)c->g.Vh;
-    const int nblk = (int)((V + HB_BLOCK - 1) / HB_BLOCK);
+    const int nblk = (c->g.Vh + HB_BLOCK - 1) / HB_BLOCK;
     double* partial = static_cast<double*>(workspace);
-    double* total = reinterpret_cast<double*>(static_cast<char*>(workspace) + align256((size_t)nblk * sizeof(double)));
-    plaquette_kernel<<<nblk, HB_BLOCK, 0, st>>>((const double*)links, c->g, partial);
+    double* total = reinterpret_cast<double*>(static_cast<char*>(workspace) + align256((size_t)2 * nblk * sizeof(double)));
+    plaquette_kernel<<<dim3(nblk, 2), HB_BLOCK, 0, st>>>((const double2*)links, c->g, partial);
     lqcd_status s = after_launch();
     if (s != LQCD_OK) return s;
-    sum_partials_kernel<<<1, BLAS_BLOCK, 0, st>>>(partial, nblk, total);
+    sum_partials_kernel<<<1, BLAS_BLOCK, 0, st>>>(partial, 2 * nblk, total);
     if ((s = after_launch()) != LQCD_OK) return s;
     double sum = 0.0;
     cudaError_t e;
     if ((e = cudaMemcpyAsync(&sum, total, sizeof(double), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
     if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
-    *plaq_host = sum / (3.0 * 6.0 * (double)V);
+    *plaq_host = sum / (3.0 * 6.0 * 2.0 * (double)c->g.Vh);
     return LQCD_OK;
 }
 

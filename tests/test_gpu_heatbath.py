@@ -1,4 +1,4 @@
-"""GPU parity of the pure-gauge heatbath (lqcd_heatbath_sublattice, lqcd_plaquette; next row f4) against
+"""GPU parity of the pure-gauge heatbath (lqcd_heatbath_sublattice, lqcd_plaquette, lqcd_pack/unpack_update_links; next row f4) against
 oracle/heatbath_oracle.py on the same links and the same uniforms: every link of the field after each of the eight
 sublattice updates, to fp64 rounding (the accept / reject decisions are taken in fp64 on both sides; a decision closer
 to its threshold than the 1e-15 the two libms differ by has probability ~1e-15 per attempt)."""
@@ -20,28 +20,48 @@ def _setup(dims, seed):
     return L, ctx, U, dev
 
 
+class _Links:
+    """A link field on the device in the update layout, converted from / to canonical numpy arrays."""
+
+    def __init__(self, ctx, U, dev):
+        self.ctx, self.dev, self.shape = ctx, dev, U.shape
+        self.buf = torch.empty(ctx.update_links_bytes(), dtype=torch.uint8, device=dev)
+        self.put(U)
+
+    def put(self, U):
+        self.ctx.pack_update_links(self.buf, torch.from_numpy(np.ascontiguousarray(U)).to(self.dev))
+        torch.cuda.synchronize()
+
+    def get(self):
+        c = torch.empty(self.shape, dtype=torch.complex128, device=self.dev)
+        self.ctx.unpack_update_links(c, self.buf)
+        torch.cuda.synchronize()
+        return c.cpu().numpy()
+
+
 @pytest.mark.parametrize("dims,beta,ntries", [((4, 4, 4, 4), 5.7, 6), ((4, 6, 8, 10), 2.0, 3), ((8, 8, 8, 16), 6.0, 4), ((6, 4, 4, 8), 0.8, 1)])
 def test_heatbath_sweep_matches_oracle(dims, beta, ntries):
     L, ctx, U, dev = _setup(dims, 61)
     Vh = ctx.Vh
     assert ctx.heatbath_uniforms(ntries) == Vh * 3 * (4 * ntries + 2)
-    Ud = torch.from_numpy(U.copy()).to(dev)
+    Ud = _Links(ctx, U, dev)
+    assert np.array_equal(Ud.get(), U)           # pack / unpack is a pure permutation
     ws = torch.empty(ctx.plaquette_workspace_bytes(), dtype=torch.uint8, device=dev)
-    assert abs(ctx.plaquette(Ud, ws) - hb.plaquette(U)) <= 1e-13
+    assert abs(ctx.plaquette(Ud.buf, ws) - hb.plaquette(U)) <= 1e-13
     rng = np.random.default_rng(5)
     changed_subgroups = 0
     for mu in range(4):
         for parity in (0, 1):
             u = 1.0 - rng.random((Vh, 3, 4 * ntries + 2))
             ref = hb.heatbath_sublattice(U, beta, mu, parity, u)
-            ctx.heatbath_sublattice(Ud, beta, mu, parity, torch.from_numpy(u).to(dev), ntries)
-            got = Ud.cpu().numpy()
+            ctx.heatbath_sublattice(Ud.buf, beta, mu, parity, torch.from_numpy(u).to(dev), ntries)
+            got = Ud.get()
             assert np.abs(got - ref).max() <= 1e-12, (mu, parity, np.abs(got - ref).max())
             changed_subgroups += int((np.abs(ref[mu] - U[mu]).reshape(-1, 9).max(axis=1) > 0).sum())
             U = ref          # the oracle's field is the reference the next update starts from on both sides
-            Ud.copy_(torch.from_numpy(U))
+            Ud.put(U)
     assert changed_subgroups > 0
-    assert abs(ctx.plaquette(Ud, ws) - hb.plaquette(U)) <= 1e-13
+    assert abs(ctx.plaquette(Ud.buf, ws) - hb.plaquette(U)) <= 1e-13
     # still SU(3)
     M = U.reshape(-1, 3, 3)
     assert np.allclose(M @ np.conj(np.swapaxes(M, -1, -2)), np.eye(3), atol=1e-12)
@@ -52,7 +72,7 @@ def test_heatbath_free_running_plaquette():
     plaquette moves from the random start (0) towards the beta = 6 value."""
     dims, beta, ntries = (4, 4, 4, 8), 6.0, 4
     L, ctx, U, dev = _setup(dims, 62)
-    Ud = torch.from_numpy(U.copy()).to(dev)
+    Ud = _Links(ctx, U, dev)
     ws = torch.empty(ctx.plaquette_workspace_bytes(), dtype=torch.uint8, device=dev)
     rng = np.random.default_rng(8)
     for sweep in range(8):
@@ -60,9 +80,9 @@ def test_heatbath_free_running_plaquette():
             for parity in (0, 1):
                 u = 1.0 - rng.random((ctx.Vh, 3, 4 * ntries + 2))
                 U = hb.heatbath_sublattice(U, beta, mu, parity, u)
-                ctx.heatbath_sublattice(Ud, beta, mu, parity, torch.from_numpy(u).to(dev), ntries)
-    assert np.abs(Ud.cpu().numpy() - U).max() <= 1e-10
-    p = ctx.plaquette(Ud, ws)
+                ctx.heatbath_sublattice(Ud.buf, beta, mu, parity, torch.from_numpy(u).to(dev), ntries)
+    assert np.abs(Ud.get() - U).max() <= 1e-10
+    p = ctx.plaquette(Ud.buf, ws)
     assert abs(p - hb.plaquette(U)) <= 1e-12 and 0.4 < p < 0.7
 
 
@@ -70,7 +90,8 @@ def test_heatbath_error_codes():
     import paper_1112_5280_b200 as L
     dims = (4, 4, 4, 4)
     _, ctx, U, dev = _setup(dims, 63)
-    Ud = torch.from_numpy(U.copy()).to(dev)
+    links = _Links(ctx, U, dev)
+    Ud = links.buf
     u = torch.rand(ctx.heatbath_uniforms(2), dtype=torch.float64, device=dev)
     for kw, status in ((dict(mu=4), L.LQCD_EINVAL), (dict(parity=2), L.LQCD_EINVAL), (dict(ntries=0), L.LQCD_EINVAL),
                        (dict(beta=0.0), L.LQCD_EINVAL)):
@@ -86,4 +107,4 @@ def test_heatbath_error_codes():
     with pytest.raises(L.LqcdError) as e:
         c32.heatbath_sublattice(Ud, 5.0, 0, 0, u, 2)
     assert e.value.status == L.LQCD_EUNSUPPORTED
-    assert np.array_equal(Ud.cpu().numpy(), U)   # nothing was launched
+    assert np.array_equal(links.get(), U)   # nothing was launched
