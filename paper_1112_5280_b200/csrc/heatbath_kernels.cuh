@@ -27,7 +27,7 @@ namespace lqcd {
 constexpr int HB_BLOCK = 128;
 // resident blocks per SM promised to ptxas for the heatbath kernel (register budget 65536 / (128 x value))
 #ifndef LQCD_HB_MINB
-#define LQCD_HB_MINB 3
+#define LQCD_HB_MINB 4
 #endif
 
 struct Mat3 { double re[9], im[9]; };   // row-major: element (r, c) at 3 r + c
@@ -68,6 +68,64 @@ __device__ __forceinline__ void mul(const Mat3& a, const Mat3& b, Mat3& c) {
             c.re[3 * r + s] = xr;
             c.im[3 * r + s] = xi;
         }
+}
+
+// Register-lean forms of the staple products (five live 3x3 complex matrices are 180 registers; these keep at most
+// three): the left / right operand is streamed from memory row by row instead of being held whole.
+//   t = op(A) m2^+  with A read from memory: row r of op(A) (a column of A if ADJA) is loaded, used, dropped
+template <bool ADJA>
+__device__ __forceinline__ void mul_streamA_adjB(const double2* links, int ntiles, int mu, int p, int cb, const Mat3& m2, Mat3& t) {
+    const double2* q = links + update_word0(ntiles, mu, p, cb);
+    const size_t Vp = (size_t)TILE * ntiles;
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        double ar[3], ai[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double2 z = __ldg(q + (ADJA ? 3 * k + r : 3 * r + k) * Vp);
+            ar[k] = z.x;
+            ai[k] = ADJA ? -z.y : z.y;
+        }
+#pragma unroll
+        for (int s2 = 0; s2 < 3; ++s2) {
+            double xr = 0.0, xi = 0.0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {   // times conj(m2[s2][k])
+                const double br = m2.re[3 * s2 + k], bi = -m2.im[3 * s2 + k];
+                xr = fma(ar[k], br, xr); xr = fma(-ai[k], bi, xr);
+                xi = fma(ar[k], bi, xi); xi = fma(ai[k], br, xi);
+            }
+            t.re[3 * r + s2] = xr;
+            t.im[3 * r + s2] = xi;
+        }
+    }
+}
+//   a += t op(B)  with B read from memory: column s of op(B) (a row of B if ADJB) is loaded, used, dropped
+template <bool ADJB>
+__device__ __forceinline__ void addmul_streamB(Mat3& a, const Mat3& t, const double2* links, int ntiles, int mu, int p, int cb) {
+    const double2* q = links + update_word0(ntiles, mu, p, cb);
+    const size_t Vp = (size_t)TILE * ntiles;
+#pragma unroll
+    for (int s2 = 0; s2 < 3; ++s2) {
+        double br[3], bi[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const double2 z = __ldg(q + (ADJB ? 3 * s2 + k : 3 * k + s2) * Vp);
+            br[k] = z.x;
+            bi[k] = ADJB ? -z.y : z.y;
+        }
+#pragma unroll
+        for (int r = 0; r < 3; ++r) {
+            double xr = a.re[3 * r + s2], xi = a.im[3 * r + s2];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                xr = fma(t.re[3 * r + k], br[k], xr); xr = fma(-t.im[3 * r + k], bi[k], xr);
+                xi = fma(t.re[3 * r + k], bi[k], xi); xi = fma(t.im[3 * r + k], br[k], xi);
+            }
+            a.re[3 * r + s2] = xr;
+            a.im[3 * r + s2] = xi;
+        }
+    }
 }
 
 // One Cabibbo-Marinari step in the block (I, J) on the link u with staple sum a: u <- G u.
@@ -146,24 +204,16 @@ __global__ void __launch_bounds__(HB_BLOCK, LQCD_HB_MINB) heatbath_kernel(double
     // nothing this launch writes
     for (int nu = 0; nu < 4; ++nu) {
         if (nu == mu) continue;
-        Mat3 m1, m2, t;
+        Mat3 m2, t;
         // upper staple  U_nu(x+mu) U_mu(x+nu)^+ U_nu(x)^+
-        load_mat(links, nt, nu, q, xmu, m1);
         load_mat(links, nt, mu, q, neighbour_rt(g, cb, s, 2 * nu), m2);
-        mul<false, true>(m1, m2, t);
-        load_mat(links, nt, nu, p, cb, m1);
-        mul<false, true>(t, m1, m2);
-#pragma unroll
-        for (int k = 0; k < 9; ++k) { a.re[k] += m2.re[k]; a.im[k] += m2.im[k]; }
+        mul_streamA_adjB<false>(links, nt, nu, q, xmu, m2, t);
+        addmul_streamB<true>(a, t, links, nt, nu, p, cb);
         // lower staple  U_nu(x+mu-nu)^+ U_mu(x-nu)^+ U_nu(x-nu)
         const int xdn = neighbour_rt(g, cb, s, 2 * nu + 1);       // x - nu^, parity q
-        load_mat(links, nt, nu, p, neighbour_rt(g, xmu, smu, 2 * nu + 1), m1);   // x + mu^ - nu^, parity p
         load_mat(links, nt, mu, q, xdn, m2);
-        mul<true, true>(m1, m2, t);
-        load_mat(links, nt, nu, q, xdn, m1);
-        mul<false, false>(t, m1, m2);
-#pragma unroll
-        for (int k = 0; k < 9; ++k) { a.re[k] += m2.re[k]; a.im[k] += m2.im[k]; }
+        mul_streamA_adjB<true>(links, nt, nu, p, neighbour_rt(g, xmu, smu, 2 * nu + 1), m2, t);   // x + mu^ - nu^, parity p
+        addmul_streamB<false>(a, t, links, nt, nu, q, xdn);
     }
     Mat3 u;
     load_mat<false>(links, nt, mu, p, cb, u);
