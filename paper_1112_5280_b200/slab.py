@@ -145,6 +145,12 @@ class SendRecvTransport:
         self.send_up, self.send_down, self.from_up, self.from_down = mk(), mk(), mk(), mk()
         self.side = torch.cuda.Stream(self.device) if self.cuda else None
         self.use_tags = dist is not None and dist.get_backend() != "nccl"
+        # a backend without device buffers (gloo: the functional test of the N > 1 path on a one-GPU box) goes through
+        # pinned host copies; NCCL sends and receives the device buffers directly
+        self.host_staged = self.cuda and dist is not None and dist.get_backend() != "nccl"
+        if self.host_staged:
+            hk = lambda: torch.zeros(hb, dtype=torch.uint8).pin_memory()
+            self.h_send_up, self.h_send_down, self.h_from_up, self.h_from_down = hk(), hk(), hk(), hk()
 
     def exchange(self, slab):
         """send_down -> rank below (its from_up), send_up -> rank above (its from_down).  On a ring of two both
@@ -157,12 +163,22 @@ class SendRecvTransport:
             self.from_down.copy_(self.send_up)
             return
         tag = (lambda t: dict(tag=t)) if self.use_tags else (lambda t: {})
-        ops = [dist.P2POp(dist.isend, self.send_down, slab.below(), **tag(self.TAG_DOWNWARD)),
-               dist.P2POp(dist.isend, self.send_up, slab.above(), **tag(self.TAG_UPWARD)),
-               dist.P2POp(dist.irecv, self.from_up, slab.above(), **tag(self.TAG_DOWNWARD)),
-               dist.P2POp(dist.irecv, self.from_down, slab.below(), **tag(self.TAG_UPWARD))]
+        sd, su, fu, fd = self.send_down, self.send_up, self.from_up, self.from_down
+        if self.host_staged:
+            import torch
+            self.h_send_down.copy_(sd, non_blocking=True)
+            self.h_send_up.copy_(su, non_blocking=True)
+            torch.cuda.current_stream(self.device).synchronize()
+            sd, su, fu, fd = self.h_send_down, self.h_send_up, self.h_from_up, self.h_from_down
+        ops = [dist.P2POp(dist.isend, sd, slab.below(), **tag(self.TAG_DOWNWARD)),
+               dist.P2POp(dist.isend, su, slab.above(), **tag(self.TAG_UPWARD)),
+               dist.P2POp(dist.irecv, fu, slab.above(), **tag(self.TAG_DOWNWARD)),
+               dist.P2POp(dist.irecv, fd, slab.below(), **tag(self.TAG_UPWARD))]
         for req in dist.batch_isend_irecv(ops):
             req.wait()
+        if self.host_staged:
+            self.from_up.copy_(fu, non_blocking=True)
+            self.from_down.copy_(fd, non_blocking=True)
 
     def push(self, slab, inp, stream):
         import torch
@@ -226,6 +242,10 @@ class PeerMemoryTransport:
         pass
 
 
+def _p2p_name(dist):
+    return "ncclSend/ncclRecv" if dist.get_backend() == "nccl" else f"{dist.get_backend()} send/recv through pinned host copies (functional test path)"
+
+
 def make_transport(slab, dist, device, kind="auto"):
     """kind: "peer" (symmetric memory, fails loudly if unavailable), "sendrecv", or "auto" (peer memory if the process
     group and the devices support it, else send/recv).  Returns (transport, name)."""
@@ -236,5 +256,5 @@ def make_transport(slab, dist, device, kind="auto"):
             if kind == "peer":
                 raise
             why = f"{type(e).__name__}: {e}"
-            return SendRecvTransport(slab, dist, device), f"ncclSend/ncclRecv (peer memory unavailable: {why[:120]})"
-    return SendRecvTransport(slab, dist, device), "ncclSend/ncclRecv"
+            return SendRecvTransport(slab, dist, device), f"{_p2p_name(dist)} (peer memory unavailable: {why[:120]})"
+    return SendRecvTransport(slab, dist, device), _p2p_name(dist)
