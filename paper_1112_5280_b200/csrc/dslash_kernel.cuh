@@ -327,6 +327,9 @@ __device__ __forceinline__ void hop_step(typename Compute<S>::type acc[24],
 #ifndef LQCD_SHFL_X
 #define LQCD_SHFL_X 0
 #endif
+#ifndef LQCD_PREFETCH_TILE_LINKS
+#define LQCD_PREFETCH_TILE_LINKS 0
+#endif
 
 template <typename R>
 __device__ __forceinline__ R shfl_(R v, int src) { return __shfl_sync(0xffffffffu, v, src); }
@@ -502,6 +505,12 @@ dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restr
     const auto* site_links = reinterpret_cast<const typename LinkStore<S, RECON>::word*>(gauge) +
                              LinkStore<S, RECON>::word0(g.ntiles, p, cb, 0);
 
+#if LQCD_PREFETCH_TILE_LINKS   // experiment: one bulk L2 prefetch of the warp tile's whole link block (8 hops, contiguous) up front
+    if ((threadIdx.x & 31u) == 0) {
+        constexpr unsigned bytes = 8u * (RECON == RECON_12H ? 12 : RECON) / LinkStore<S, RECON>::R_PER_WORD * TILE * sizeof(typename LinkStore<S, RECON>::word);
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(site_links), "r"(bytes) : "memory");
+    }
+#endif
     R acc[24];
 #pragma unroll
     for (int k = 0; k < 24; ++k) acc[k] = 0;

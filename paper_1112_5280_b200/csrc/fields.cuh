@@ -405,11 +405,13 @@ __host__ __device__ __forceinline__ size_t half_stride(int ntiles) {
 template <typename S, int RECON> struct LinkStore {
     using R = typename Compute<S>::type;
     using word = typename LinkWord<R, RECON>::type;
+    static constexpr int R_PER_WORD = LinkWord<R, RECON>::LW;
     static __host__ __device__ __forceinline__ size_t word0(int ntiles, int p, int cb, int k) { return link_word0<R, RECON>(ntiles, p, cb, k); }
 };
 template <int RECON> struct LinkStore<__half, RECON> {
     using R = float;
     using word = uint2;
+    static constexpr int R_PER_WORD = 4;
     static __host__ __device__ __forceinline__ size_t word0(int ntiles, int p, int cb, int k) { return link_word0_h(ntiles, p, cb, k); }
 };
 // fp32 spinors with the links stored as 12 halfs (lqcd_params.link_precision = 16): the link stream is 2/3 of
@@ -418,6 +420,7 @@ constexpr int RECON_12H = 13;
 template <> struct LinkStore<float, RECON_12H> {
     using R = float;
     using word = uint2;
+    static constexpr int R_PER_WORD = 4;
     static __host__ __device__ __forceinline__ size_t word0(int ntiles, int p, int cb, int k) { return link_word0_h(ntiles, p, cb, k); }
 };
 template <typename S, int RECON> constexpr bool half_links = sizeof(S) == 2 || RECON == RECON_12H;
