@@ -279,6 +279,10 @@ lqcd_status lqcd_plaquette(const lqcd_ctx* ctx, const void* links_update_dev, vo
                                  (every warp double-buffers its tile's link blocks with cp.async.bulk); precision 32 / 64 */
 lqcd_status lqcd_set_kernel(lqcd_ctx* ctx, int kernel);
 
+/* Host-side self test of the index map's division-free arithmetic: n / d as the kernels compute it (multiply-shift by a
+ * reciprocal of the extent d set up in lqcd_create), for 1 <= d and n < 2^30.  tests/test_abi.py compares it with n / d. */
+unsigned lqcd_selftest_fastdiv(unsigned d, unsigned n);
+
 /* Number of kernels this library has launched since load (a claim counter for bench.py). */
 unsigned long long lqcd_launch_count(void);
 

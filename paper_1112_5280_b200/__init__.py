@@ -21,7 +21,7 @@ EXPORTS = [
     "lqcd_create", "lqcd_destroy", "lqcd_spinor_bytes", "lqcd_gauge_bytes", "lqcd_workspace_bytes",
     "lqcd_host_workspace_bytes", "lqcd_pack_gauge", "lqcd_pack_spinor", "lqcd_unpack_spinor",
     "lqcd_dslash_full", "lqcd_dslash_eo", "lqcd_apply_M", "lqcd_set_time_slab", "lqcd_dslash_eo_range", "lqcd_pack_gauge_slab", "lqcd_halo_bytes", "lqcd_slab_push_faces", "lqcd_dslash_eo_slab", "lqcd_apply_M_tm", "lqcd_apply_Q_tm", "lqcd_cg_workspace_bytes", "lqcd_cg_solve_tm", "lqcd_cg_mixed_workspace_bytes", "lqcd_cg_solve_tm_mixed", "lqcd_dslash_eo_host", "lqcd_dslash_eo_host_batch", "lqcd_launch_count",
-    "lqcd_gauge_recon8_margin", "lqcd_set_kernel", "lqcd_update_links_bytes", "lqcd_pack_update_links", "lqcd_unpack_update_links",
+    "lqcd_gauge_recon8_margin", "lqcd_set_kernel", "lqcd_selftest_fastdiv", "lqcd_update_links_bytes", "lqcd_pack_update_links", "lqcd_unpack_update_links",
     "lqcd_heatbath_uniforms", "lqcd_heatbath_sublattice",
     "lqcd_plaquette_workspace_bytes", "lqcd_plaquette", "lqcd_status_string", "lqcd_last_cuda_error",
 ]
@@ -68,6 +68,8 @@ def _lib():
         lib.lqcd_apply_M.argtypes = [vp, vp, vp, vp, cd, ci, vp, vp]
         lib.lqcd_set_time_slab.argtypes = [vp, ci, ci]
         lib.lqcd_set_kernel.argtypes = [vp, ci]
+        lib.lqcd_selftest_fastdiv.argtypes = [ctypes.c_uint, ctypes.c_uint]
+        lib.lqcd_selftest_fastdiv.restype = ctypes.c_uint
         lib.lqcd_update_links_bytes.argtypes = [vp]
         lib.lqcd_update_links_bytes.restype = sz
         lib.lqcd_pack_update_links.argtypes = [vp, vp, vp, vp]

@@ -32,7 +32,7 @@ inline void set_fastdiv(unsigned d, unsigned& mul, int& shift) {
     shift = 30 + l;
     mul = (unsigned)((((unsigned long long)1 << shift) + d - 1) / d);
 }
-__device__ __forceinline__ unsigned fastdiv(unsigned n, unsigned mul, int shift) {
+__host__ __device__ __forceinline__ unsigned fastdiv(unsigned n, unsigned mul, int shift) {
     return (unsigned)(((unsigned long long)n * mul) >> shift);
 }
 

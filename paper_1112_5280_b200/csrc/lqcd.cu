@@ -761,6 +761,13 @@ lqcd_status lqcd_plaquette(const lqcd_ctx* c, const void* links, void* workspace
     return LQCD_OK;
 }
 
+unsigned lqcd_selftest_fastdiv(unsigned d, unsigned n) {
+    unsigned mul;
+    int shift;
+    set_fastdiv(d, mul, shift);
+    return fastdiv(n, mul, shift);
+}
+
 unsigned long long lqcd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 const char* lqcd_status_string(lqcd_status s) {

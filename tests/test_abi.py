@@ -88,3 +88,20 @@ def test_alignment_contract_checked_before_any_launch():
         assert lib.lqcd_pack_spinor(c._h, base, far + 8, 0, None) == L.LQCD_EALIGN            # canonical side: 16
         assert lib.lqcd_unpack_spinor(c._h, far + 8, base, 0, None) == L.LQCD_EALIGN
     assert b"32" in lib.lqcd_status_string(L.LQCD_EALIGN)
+
+
+def test_division_free_index_map_equals_integer_division():
+    """decode_site divides checkerboard indices (< 2^30) by the run-time extents with a multiply-shift (geometry.cuh);
+    the library's own routine, on the host, against n // d: every extent up to 600, large and awkward ones, indices at
+    both ends of the range, around multiples of d, and random."""
+    import numpy as np
+    lib = L._lib()
+    rng = np.random.default_rng(0)
+    for d in list(range(1, 601)) + [1023, 1024, 1025, 4097, 65535, 65536, 65537, 100003, (1 << 20) - 1, (1 << 24) + 5, (1 << 29) + 1]:
+        ns = set(int(x) for x in rng.integers(0, 1 << 30, 40))
+        ns |= {0, 1, d - 1, d, d + 1, (1 << 30) - 1, (1 << 30) - d, ((1 << 30) // d) * d - 1, ((1 << 30) // d) * d}
+        for k in (3, 1000, 123457):
+            ns |= {k * d - 1, k * d, k * d + 1}
+        for n in ns:
+            if 0 <= n < (1 << 30):
+                assert lib.lqcd_selftest_fastdiv(d, n) == n // d, (d, n)
