@@ -318,15 +318,16 @@ def test_half_precision_storage(H, dims, bc):
     assert not g.dslash_eo(z, 0).any()
 
 
-@pytest.mark.parametrize("precision", [16, 32, 64])
-def test_no_writes_outside_the_declared_buffer_sizes(H, precision):
+@pytest.mark.parametrize("precision,kernel", [(16, "gather"), (32, "gather"), (64, "gather"), (32, "pipe"), (64, "pipe"),
+                                              (32, "lstage"), (64, "lstage"), (32, "blocked")])
+def test_no_writes_outside_the_declared_buffer_sizes(H, precision, kernel):
     """Every output / workspace buffer is carved out of a larger allocation filled with a canary byte; after the
     hot-path calls on a lattice with a ragged last tile, everything outside the declared sizes is untouched."""
     import torch
     dims, bc = (6, 6, 6, 6), (1, 1, 1, -1)
     U = li.random_su3_links(dims, seed=95).astype(H.cdtype(precision))
     psi = li.gaussian_spinor(dims, seed=96).astype(H.cdtype(precision))
-    g = H.Gpu(dims, precision, 12, bc, U)
+    g = H.Gpu(dims, precision, 12, bc, U, kernel=kernel)
     G = 4096
     def guarded(nbytes):
         big = torch.full((nbytes + 2 * G,), 0xAB, dtype=torch.uint8, device="cuda:0")
