@@ -165,3 +165,23 @@ def test_largest_lattice_index_headroom():
         ref = oracle.dslash_sites(U, psi, dims, bc, sites)
         H.assert_parity(got[cb_index(dims, sites)], ref, 32)
         assert np.isfinite(got.view(np.float32)).all()
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("kernel", ["pipe", "lstage", "blocked"])
+def test_config4_kernel_variants_bitwise(cfg4, precision, kernel):
+    """At the bench size (32^3 x 64: 32768 warp tiles per parity, ~220 per persistent CTA) the data-movement variants
+    of lqcd_set_kernel give the gather kernel's result bit for bit, both parities; the gather kernel itself is checked
+    against the oracle on sampled sites above."""
+    import gpu_harness as H
+    c, U64, psi64 = cfg4
+    dims, bc = c["dims"], c["bc"]
+    U = U64.astype(H.cdtype(precision))
+    psi = psi64.astype(H.cdtype(precision))
+    ref = H.Gpu(dims, precision, 12, bc, U, kernel="gather")
+    g = H.Gpu(dims, precision, 12, bc, U, kernel=kernel)
+    for out_parity in (0, 1):
+        half = H.half_of(psi, dims, 1 - out_parity)
+        assert np.array_equal(g.dslash_eo(half, out_parity), ref.dslash_eo(half, out_parity)), (kernel, precision, out_parity)
+    e = H.half_of(psi, dims, 0)
+    assert np.array_equal(g.apply_M(e, c["kappa"], 1, mu=0.1), ref.apply_M(e, c["kappa"], 1, mu=0.1))
