@@ -52,9 +52,26 @@ template <typename R> struct BcPhases { R re[4], im[4]; };
 
 // K3: half spinor h[spin 2][colour 3][reim] = the upper two components of (1 -+ gamma_mu) psi for the forward /
 // backward hop (S = +1 / -1), from a gathered neighbour spinor v.
+// a + C b for a unit coefficient C on packed complex numbers
+template <int C>
+__device__ __forceinline__ P2 cadd2(float ar, float ai, float br, float bi) {
+    if (C == C_P1) return add2(pk(ar, ai), pk(br, bi));
+    if (C == C_M1) return add2(pk(ar, ai), pk(-br, -bi));
+    if (C == C_PI) return add2(pk(ar, ai), pk(-bi, br));
+    return add2(pk(ar, ai), pk(bi, -br));
+}
+
 template <typename R, int MU, int S>
 __device__ __forceinline__ void project(const R v[24], R h[12]) {
     using P = Proj<MU>;
+    if constexpr (packed_f32<R>) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            unpk(cadd2<coef_sgn<S>(P::ca)>(v[2 * c], v[2 * c + 1], v[6 * P::ja + 2 * c], v[6 * P::ja + 2 * c + 1]), h[2 * c], h[2 * c + 1]);
+            unpk(cadd2<coef_sgn<S>(P::cb)>(v[6 + 2 * c], v[6 + 2 * c + 1], v[6 * P::jb + 2 * c], v[6 * P::jb + 2 * c + 1]), h[6 + 2 * c], h[6 + 2 * c + 1]);
+        }
+        return;
+    }
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         R r0 = v[2 * c], i0 = v[2 * c + 1];
@@ -118,6 +135,28 @@ __device__ __forceinline__ R boundary_phase(R h[12], R scale, bool cross, R br, 
 // K4: chi = U h (forward) or U^+ h (backward), both spin components; explicit FMA chains
 template <typename R, bool FWD>
 __device__ __forceinline__ void su3_multiply(const R h[12], const R u[18], R chi[12]) {
+    if constexpr (packed_f32<R>) {
+        // (re, im) as one pair: P = sum_b ur (hr, hi), Q = sum_b ui (hi, hr); forward chi = (P.x - Q.x, P.y + Q.y),
+        // backward (conjugated link) chi = (P.x + Q.x, P.y - Q.y): 2 FFMA2 per complex multiply-add, 1 FADD2 per output
+#pragma unroll
+        for (int sp = 0; sp < 2; ++sp)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                P2 pp, qq;
+#pragma unroll
+                for (int b = 0; b < 3; ++b) {
+                    const float hr = h[6 * sp + 2 * b], hi = h[6 * sp + 2 * b + 1];
+                    const float ur = FWD ? u[6 * a + 2 * b] : u[6 * b + 2 * a];
+                    const float ui = FWD ? u[6 * a + 2 * b + 1] : u[6 * b + 2 * a + 1];
+                    pp = b == 0 ? mul2(bc2(ur), pk(hr, hi)) : fma2(bc2(ur), pk(hr, hi), pp);
+                    qq = b == 0 ? mul2(bc2(ui), pk(hi, hr)) : fma2(bc2(ui), pk(hi, hr), qq);
+                }
+                float qx, qy;
+                unpk(qq, qx, qy);
+                unpk(add2(pp, FWD ? pk(-qx, qy) : pk(qx, -qy)), chi[6 * sp + 2 * a], chi[6 * sp + 2 * a + 1]);
+            }
+        return;
+    }
 #pragma unroll
     for (int sp = 0; sp < 2; ++sp)
 #pragma unroll
@@ -145,9 +184,30 @@ __device__ __forceinline__ void su3_multiply(const R h[12], const R u[18], R chi
 }
 
 // K5: out0 += f chi0, out1 += f chi1, out2 += f S c2 chi_k2, out3 += f S c3 chi_k3
+// d += f c s for a unit coefficient c, packed
+template <int C>
+__device__ __forceinline__ void cfma2(float& dr, float& di, float f, float sr, float si) {
+    P2 d = pk(dr, di);
+    if (C == C_P1) d = fma2(bc2(f), pk(sr, si), d);
+    else if (C == C_M1) d = fma2(bc2(-f), pk(sr, si), d);
+    else if (C == C_PI) d = fma2(pk(-f, f), pk(si, sr), d);    // dr += -f si, di += f sr
+    else d = fma2(pk(f, -f), pk(si, sr), d);                   // dr += f si, di += -f sr
+    unpk(d, dr, di);
+}
+
 template <typename R, int MU, int S>
 __device__ __forceinline__ void reconstruct_accumulate(R acc[24], const R chi[12], R f) {
     using P = Proj<MU>;
+    if constexpr (packed_f32<R>) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            cfma2<C_P1>(acc[2 * c], acc[2 * c + 1], f, chi[2 * c], chi[2 * c + 1]);
+            cfma2<C_P1>(acc[6 + 2 * c], acc[6 + 2 * c + 1], f, chi[6 + 2 * c], chi[6 + 2 * c + 1]);
+            cfma2<coef_sgn<S>(P::c2)>(acc[12 + 2 * c], acc[12 + 2 * c + 1], f, chi[6 * P::k2 + 2 * c], chi[6 * P::k2 + 2 * c + 1]);
+            cfma2<coef_sgn<S>(P::c3)>(acc[18 + 2 * c], acc[18 + 2 * c + 1], f, chi[6 * P::k3 + 2 * c], chi[6 * P::k3 + 2 * c + 1]);
+        }
+        return;
+    }
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         acc[2 * c] = fma_(f, chi[2 * c], acc[2 * c]);

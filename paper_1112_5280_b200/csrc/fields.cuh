@@ -178,6 +178,26 @@ __device__ __forceinline__ float2  ld_stream(const float2* p)  { return __ldcs(p
 __device__ __forceinline__ double2 ld_stream(const double2* p) { return __ldcs(p); }
 __device__ __forceinline__ double4_ ld_stream(const double4_* p) { return ldg256_stream(p); }
 
+// Packed fp32 arithmetic (Blackwell FFMA2 / FMUL2 / FADD2: two fp32 operations per instruction on an aligned register
+// pair).  A complex number is one pair (re low, im high).  The SASS operand modifiers make a complex multiply-add two
+// instructions with no data movement: a scalar operand is broadcast to both lanes (.F32), a pair can be read swapped
+// (.LO_HI), and FADD2 can negate one half (.NP), so a complex sum  sum_b u_b z_b  is  P = sum ur (zr, zi),
+// Q = sum ui (zi, zr)  (two FFMA2 per term)  and  (P.x - Q.x, P.y + Q.y)  (one FADD2).
+// Each lane is an IEEE operation; the real and the imaginary-unit parts of a complex sum are accumulated in two
+// chains and combined at the end (FFMA2 can negate a whole operand, FADD2 also one half of it), so the rounding order
+// differs from the scalar code in the last bit -- every fp32 kernel variant shares these routines.
+#ifndef LQCD_FFMA2
+#define LQCD_FFMA2 1
+#endif
+struct P2 { unsigned long long v; };
+__device__ __forceinline__ P2 pk(float lo, float hi) { P2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void unpk(P2 p, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(p.v)); }
+__device__ __forceinline__ P2 fma2(P2 a, P2 b, P2 c) { P2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return d; }
+__device__ __forceinline__ P2 mul2(P2 a, P2 b) { P2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
+__device__ __forceinline__ P2 add2(P2 a, P2 b) { P2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v)); return d; }
+__device__ __forceinline__ P2 bc2(float s) { return pk(s, s); }
+template <typename R> constexpr bool packed_f32 = LQCD_FFMA2 && sizeof(R) == 4;
+
 // K2: rebuild row 2 of u[18] (row-major 3x3 complex, u[6 row + 2 col + reim]) as conj(row0 x row1);
 // valid for det U = +1 ("RECONSTRUCT TWELVE").
 template <typename R>
@@ -188,6 +208,20 @@ __device__ __forceinline__ void recon_row2(R u[18]) {
         const int a = (c + 1) % 3, b = (c + 2) % 3;
         const R ar = u[2 * a], ai = u[2 * a + 1], br = u[2 * b], bi = u[2 * b + 1];
         const R cr = u[6 + 2 * b], ci = u[6 + 2 * b + 1], dr = u[6 + 2 * a], di = u[6 + 2 * a + 1];
+        if constexpr (packed_f32<R>) {
+            // t = a c - b d with (re, im) as one pair: P = ar (cr, ci) - br (dr, di), Q = ai (ci, cr) - bi (di, dr) (swapped
+            // reads), t = (P.x - Q.x, P.y + Q.y); FFMA2 negates whole operands only, FADD2 also one half
+            P2 pp = mul2(bc2(ar), pk(cr, ci));
+            pp = fma2(bc2(-br), pk(dr, di), pp);
+            P2 qq = mul2(bc2(ai), pk(ci, cr));
+            qq = fma2(bc2(-bi), pk(di, dr), qq);
+            float qx, qy, re2, im2;
+            unpk(qq, qx, qy);
+            unpk(add2(pp, pk(-qx, qy)), re2, im2);
+            u[12 + 2 * c] = re2;
+            u[12 + 2 * c + 1] = -im2;
+            continue;
+        }
         const R re = fmar(-br, dr, fmar(bi, di, fmar(-ai, ci, ar * cr)));
         const R im = fmar(-br, di, fmar(-bi, dr, fmar(ai, cr, ar * ci)));
         u[12 + 2 * c] = re;
