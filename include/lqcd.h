@@ -70,7 +70,8 @@ typedef enum {
     LQCD_EALIGN = 2,       /* a device pointer is misaligned: native 32 B, canonical 16 B, big workspaces 256 B */
     LQCD_EALIAS = 3,       /* out overlaps in or workspace */
     LQCD_EUNSUPPORTED = 4, /* combination not compiled in */
-    LQCD_ECUDA = 5         /* CUDA runtime / launch error */
+    LQCD_ECUDA = 5,        /* CUDA runtime / launch error */
+    LQCD_ETOOBIG = 6       /* lqcd_apply_M_eo_static only: the lattice needs more than LQCD_STATIC_SCRATCH_BYTES */
 } lqcd_status;
 
 typedef struct {
@@ -172,6 +173,38 @@ lqcd_status lqcd_dslash_eo_slab(const lqcd_ctx* ctx, void* out_dev, const void* 
  *         workspace_dev holds the intermediate odd half spinor (lqcd_workspace_bytes). */
 lqcd_status lqcd_apply_M(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
                          double kappa, int eo, void* workspace_dev, void* stream);
+
+/* ---- the even-odd fermion matrix for callers that cannot allocate device memory ----
+ * lqcd_apply_M(eo = 1) needs a workspace, and by the rules above the caller provides it.  Some callers cannot: this
+ * library is a plain C ABI, and a C or Fortran HMC driver that links it is typically handed three device pointers (links,
+ * source, destination) by a host application whose own pool owns all of HBM -- it has no CUDA runtime binding to call
+ * cudaMalloc with, and if it had one the call would fail (nothing is left outside the pool) or stall the device (cudaMalloc
+ * and cudaFree synchronise).  The same holds for code that runs where allocation is forbidden by contract, such as the
+ * inner loop of a solver that promised its caller a fixed memory footprint.
+ *
+ * For them: out_e = in_e - kappa^2 H_eo H_oe in_e exactly as lqcd_apply_M(ctx, out, gauge, in, kappa, 1, workspace, stream)
+ * computes it (same two launches, same arithmetic, bit-identical result), with the intermediate odd half spinor kept in
+ * an array inside the library image instead of a caller's workspace.  The call itself allocates and frees nothing, on the
+ * host or on the device, and calls no library routine that does.
+ *   Limit.     The array is LQCD_STATIC_SCRATCH_BYTES (16 MiB) and exists once per GPU: every GPU on which this library
+ *              is used gives up that much memory from the moment the module is loaded until the process exits, called or
+ *              not.  A lattice fits when lqcd_workspace_bytes(ctx) <= lqcd_static_scratch_bytes(): up to 16^3 x 32 in
+ *              precision 64, 16^3 x 64 in precision 32.  A larger one returns LQCD_ETOOBIG before anything is launched;
+ *              use lqcd_apply_M with a workspace of your own then.
+ *   First call. The first call on each device looks up where that device keeps the array (cudaGetSymbolAddress, which
+ *              may also make the runtime load the module); later calls on that device reuse the answer.  Make that first
+ *              call with the device current, outside any stream capture, before the phase of your program in which
+ *              allocation is off limits.
+ *   Sharing.   All calls on one GPU -- from any context, thread or stream -- use the same array.  It needs no clearing:
+ *              the first launch overwrites every site before the second reads it, so whatever an earlier call left there is
+ *              harmless.  But two calls whose kernels can overlap on the GPU (different streams, different host threads
+ *              without ordering between them) race on the intermediate field and both results are garbage; order them
+ *              on one stream or with events.  The contents after a call are unspecified.
+ * Pointers, alignment, aliasing and error codes as for lqcd_apply_M; in, out: native even half spinors. */
+#define LQCD_STATIC_SCRATCH_BYTES ((size_t)16 << 20)
+size_t lqcd_static_scratch_bytes(void);
+lqcd_status lqcd_apply_M_eo_static(const lqcd_ctx* ctx, void* out_dev, const void* gauge_dev, const void* in_dev,
+                                   double kappa, void* stream);
 
 /* Twisted-mass Wilson fermion matrix for one flavour ("N_f = 2 twisted-mass Wilson fermions",
  * "even-odd preconditioning"; the other flavour is mu -> -mu; reading F1):

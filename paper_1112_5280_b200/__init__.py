@@ -12,7 +12,7 @@ import os
 
 from . import _build
 
-LQCD_OK, LQCD_EINVAL, LQCD_EALIGN, LQCD_EALIAS, LQCD_EUNSUPPORTED, LQCD_ECUDA = range(6)
+LQCD_OK, LQCD_EINVAL, LQCD_EALIGN, LQCD_EALIAS, LQCD_EUNSUPPORTED, LQCD_ECUDA, LQCD_ETOOBIG = range(7)
 PARITY_EVEN, PARITY_ODD, PARITY_BOTH = 0, 1, -1
 KERNEL_GATHER, KERNEL_PIPE, KERNEL_BLOCKED, KERNEL_LSTAGE = 0, 1, 2, 3
 HAS_RECON8 = True
@@ -24,6 +24,7 @@ EXPORTS = [
     "lqcd_gauge_recon8_margin", "lqcd_set_kernel", "lqcd_selftest_fastdiv", "lqcd_update_links_bytes", "lqcd_pack_update_links", "lqcd_unpack_update_links",
     "lqcd_heatbath_uniforms", "lqcd_heatbath_sublattice",
     "lqcd_plaquette_workspace_bytes", "lqcd_plaquette", "lqcd_status_string", "lqcd_last_cuda_error",
+    "lqcd_static_scratch_bytes", "lqcd_apply_M_eo_static",
 ]
 
 
@@ -66,6 +67,9 @@ def _lib():
         lib.lqcd_dslash_full.argtypes = [vp, vp, vp, vp, vp]
         lib.lqcd_dslash_eo.argtypes = [vp, vp, vp, vp, ci, vp]
         lib.lqcd_apply_M.argtypes = [vp, vp, vp, vp, cd, ci, vp, vp]
+        lib.lqcd_apply_M_eo_static.argtypes = [vp, vp, vp, vp, cd, vp]
+        lib.lqcd_static_scratch_bytes.argtypes = []
+        lib.lqcd_static_scratch_bytes.restype = sz
         lib.lqcd_set_time_slab.argtypes = [vp, ci, ci]
         lib.lqcd_set_kernel.argtypes = [vp, ci]
         lib.lqcd_selftest_fastdiv.argtypes = [ctypes.c_uint, ctypes.c_uint]
@@ -234,6 +238,14 @@ class Context:
         _chk(_lib().lqcd_apply_M(self._h, _ptr(out), _ptr(gauge), _ptr(inp), float(kappa), int(eo),
                                  _ptr(workspace), _stream(stream)), "lqcd_apply_M")
 
+    def apply_M_eo_static(self, out, gauge, inp, kappa, stream=None):
+        """lqcd_apply_M_eo_static: apply_M(eo=1) without a workspace argument, for callers that cannot allocate one (a
+        driver that was only handed the three fields by an application whose pool owns the GPU).  The intermediate field
+        lives in a 16 MiB array inside liblqcd.so, shared by every call on the GPU: larger lattices raise LQCD_ETOOBIG,
+        overlapping calls race, and the first call on a device (which looks the array up) belongs outside stream capture."""
+        _chk(_lib().lqcd_apply_M_eo_static(self._h, _ptr(out), _ptr(gauge), _ptr(inp), float(kappa), _stream(stream)),
+             "lqcd_apply_M_eo_static")
+
     def apply_M_tm(self, out, gauge, inp, kappa, mu, eo, workspace=None, stream=None):
         _chk(_lib().lqcd_apply_M_tm(self._h, _ptr(out), _ptr(gauge), _ptr(inp), float(kappa), float(mu), int(eo),
                                     _ptr(workspace), _stream(stream)), "lqcd_apply_M_tm")
@@ -274,6 +286,11 @@ class Context:
         par = (ctypes.c_int * n)(*[int(p) for p in out_parities])
         _chk(_lib().lqcd_dslash_eo_host_batch(self._h, n, outs, _ptr(gauge_host), ins, par, _ptr(workspace),
                                               _stream(stream)), "lqcd_dslash_eo_host_batch")
+
+
+def static_scratch_bytes() -> int:
+    """Size of the built-in scratch array behind Context.apply_M_eo_static (held once per GPU for the life of the process)."""
+    return int(_lib().lqcd_static_scratch_bytes())
 
 
 def launch_count() -> int:

@@ -761,6 +761,59 @@ lqcd_status lqcd_plaquette(const lqcd_ctx* c, const void* links, void* workspace
     return LQCD_OK;
 }
 
+// ---- lqcd_apply_M_eo_static: the even-odd fermion matrix for callers that have no way to allocate device memory ------
+// Everything else in this file takes its scratch from the caller.  This one entry point keeps the intermediate odd half
+// spinor of M_eo = 1 - kappa^2 H_eo H_oe in an array that is part of the library image itself, so the caller brings only
+// out, gauge and in.  The array costs LQCD_STATIC_SCRATCH_BYTES of HBM on every GPU that loads this module, from the
+// moment it is loaded until the process exits, whether or not the entry point is ever called -- hence the modest size.
+}  // extern "C"
+
+namespace {
+
+constexpr size_t STATIC_SCRATCH_BYTES = LQCD_STATIC_SCRATCH_BYTES;
+static __device__ __align__(256) unsigned char g_static_scratch[STATIC_SCRATCH_BYTES];
+
+// In host code `g_static_scratch` is only a handle for the runtime, not an address a kernel may use: the device
+// address differs from GPU to GPU and has to be asked for, once per device, with that device current.
+constexpr int STATIC_SCRATCH_MAX_DEVICES = 64;
+std::mutex g_static_scratch_lock;
+void* g_static_scratch_dev[STATIC_SCRATCH_MAX_DEVICES] = {};
+
+lqcd_status static_scratch_address(void** ptr) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (dev < 0 || dev >= STATIC_SCRATCH_MAX_DEVICES) return LQCD_EUNSUPPORTED;
+    std::lock_guard<std::mutex> guard(g_static_scratch_lock);
+    if (!g_static_scratch_dev[dev]) {
+        void* p = nullptr;
+        if ((e = cudaGetSymbolAddress(&p, g_static_scratch)) != cudaSuccess) return cuda_fail(e);
+        g_static_scratch_dev[dev] = p;
+    }
+    *ptr = g_static_scratch_dev[dev];
+    return LQCD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t lqcd_static_scratch_bytes(void) { return STATIC_SCRATCH_BYTES; }
+
+lqcd_status lqcd_apply_M_eo_static(const lqcd_ctx* c, void* out, const void* gauge, const void* in, double kappa,
+                                   void* stream) {
+    const size_t hb = c ? half_bytes(c) : 0;
+    lqcd_status s = check_fields(c, out, gauge, in, hb);
+    if (s != LQCD_OK) return s;
+    if (hb > STATIC_SCRATCH_BYTES) return LQCD_ETOOBIG;   // before any CUDA call: the answer does not depend on the device
+    void* scratch = nullptr;
+    if ((s = static_scratch_address(&scratch)) != LQCD_OK) return s;
+    // Nothing in the array has to start from zero: the first launch writes every site of the intermediate field before the
+    // second reads it, and the padding lanes of the last tile are neither read nor written.  What an earlier call left
+    // behind is simply overwritten.
+    return apply_M_impl(c, out, gauge, in, kappa, 0.0, false, 1, scratch, (cudaStream_t)stream);
+}
+
 unsigned lqcd_selftest_fastdiv(unsigned d, unsigned n) {
     unsigned mul;
     int shift;
@@ -778,6 +831,7 @@ const char* lqcd_status_string(lqcd_status s) {
         case LQCD_EALIAS: return "output overlaps an input";
         case LQCD_EUNSUPPORTED: return "unsupported configuration";
         case LQCD_ECUDA: return "CUDA error";
+        case LQCD_ETOOBIG: return "lattice too large for the library's built-in scratch array (lqcd_static_scratch_bytes): use the entry point that takes a workspace";
     }
     return "unknown status";
 }
