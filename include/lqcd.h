@@ -84,7 +84,8 @@ typedef struct {
                          parametrisation of ref. [3]: U01, U02, U10 and the phases of U00, U20,
                          the rest rebuilt in registers from unitarity and det = 1 (precision 32 / 64 only).
                          Singular where |U00| = 1: unit links cannot be stored with recon 8, and a link loses
-                         digits like eps / min(|U00|, sqrt(1 - |U00|^2), |U20|) -- see lqcd_gauge_recon8_margin */
+                         digits like eps / min(|U00|, sqrt(1 - |U00|^2), |U20|) -- see lqcd_gauge_recon8_margin.
+                         lqcd_pack_gauge refuses a field with a link whose margin is below 64 eps (LQCD_EUNSUPPORTED) */
     double bc_re[4];  /* boundary phase bc_mu = bc_re + i bc_im, |bc_mu| = 1 within 1e-12; */
     double bc_im[4];  /* periodic (1,0), antiperiodic (-1,0), any U(1) phase allowed        */
     int link_precision; /* 0: links stored like the spinors.  16 with precision 32 and recon 12: fp32 spinors,
@@ -110,6 +111,10 @@ size_t lqcd_host_workspace_bytes(const lqcd_ctx* ctx);   /* device scratch of lq
  * All pointers are device pointers; asynchronous on `stream`.
  * parity = LQCD_PARITY_EVEN/ODD: canonical half spinor <-> native half spinor;
  * parity = LQCD_PARITY_BOTH:     canonical full spinor <-> native full spinor [even|odd]. */
+/* recon 8 only: lqcd_pack_gauge / lqcd_pack_gauge_slab also check every link against the encoding's singular set (unit
+ * links, |U00| = 1, U00 = 0 or U20 = 0: the decoder would divide by zero and the dslash would return NaN) and, for that,
+ * synchronise `stream` before returning: LQCD_EUNSUPPORTED if a link's margin (lqcd_gauge_recon8_margin) is below
+ * 64 eps of the precision, or is NaN; the native buffer is then not usable.  Store such a field with recon 12. */
 lqcd_status lqcd_pack_gauge(const lqcd_ctx* ctx, void* native_dev, const void* canonical_dev, void* stream);
 lqcd_status lqcd_pack_spinor(const lqcd_ctx* ctx, void* native_dev, const void* canonical_dev, int parity,
                              void* stream);

@@ -170,6 +170,33 @@ size_t lqcd_host_workspace_bytes(const lqcd_ctx* c) {
            HOST_SLOTS * 2 * (align256(half_bytes(c)) + align256(canon_half));
 }
 
+// 8-real links: the pack kernel raises this flag for a link the decoder cannot rebuild.  One flag per GPU, inside the
+// library image (the library allocates nothing); g_recon8_lock keeps the clear / launch / read-back of two packs apart.
+static __device__ unsigned g_recon8_bad;
+static std::mutex g_recon8_lock;
+
+// Smallest admissible min(|U00|, sqrt(|U01|^2 + |U02|^2), |U20|) of a link stored with 8 reals: the decoder loses digits
+// like eps / margin, so below 64 eps not even two digits of the rebuilt rows are right (0: unit links, NaN).
+static double recon8_min_margin(int precision) { return 64.0 * (precision == 64 ? 0x1p-53 : 0x1p-24); }
+
+static lqcd_status pack_gauge8_checked(const lqcd_ctx* c, void* native, const void* canon, const void* below, dim3 grid,
+                                       cudaStream_t st) {
+    std::lock_guard<std::mutex> guard(g_recon8_lock);
+    unsigned* bad_dev = nullptr;
+    unsigned bad = 0;
+    cudaError_t e;
+    if ((e = cudaGetSymbolAddress((void**)&bad_dev, g_recon8_bad)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemsetAsync(bad_dev, 0, sizeof(unsigned), st)) != cudaSuccess) return cuda_fail(e);
+    const double m = recon8_min_margin(c->p.precision);
+    if (c->p.precision == 32) pack_gauge8_kernel<float><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, (const float*)below, c->g, m * m, bad_dev);
+    else pack_gauge8_kernel<double><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, (const double*)below, c->g, m * m, bad_dev);
+    lqcd_status s = after_launch();
+    if (s != LQCD_OK) return s;
+    if ((e = cudaMemcpyAsync(&bad, bad_dev, sizeof(unsigned), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+    return bad ? LQCD_EUNSUPPORTED : LQCD_OK;   // the field has a link outside the 8-real encoding: store it with 12
+}
+
 static lqcd_status pack_gauge_impl(const lqcd_ctx* c, void* native, const void* canon, const void* below, void* stream) {
     if (!c || !native || !canon) return LQCD_EINVAL;
     if (!aligned32(native) || !aligned16(canon) || !aligned16(below)) return LQCD_EALIGN;
@@ -178,8 +205,7 @@ static lqcd_status pack_gauge_impl(const lqcd_ctx* c, void* native, const void* 
     if (c->p.precision == 16 || c->p.link_precision == 16) {
         pack_gauge_h_kernel<<<grid, 128, 0, st>>>((__half*)native, (const float*)canon, (const float*)below, c->g);
     } else if (c->p.recon == 8) {
-        if (c->p.precision == 32) pack_gauge8_kernel<float><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, (const float*)below, c->g);
-        else pack_gauge8_kernel<double><<<grid, 128, 0, st>>>((double*)native, (const double*)canon, (const double*)below, c->g);
+        return pack_gauge8_checked(c, native, canon, below, grid, st);
     } else if (c->p.precision == 32) {
         if (c->p.recon == 12) pack_gauge_kernel<float, 12><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, (const float*)below, c->g);
         else pack_gauge_kernel<float, 18><<<grid, 128, 0, st>>>((float*)native, (const float*)canon, (const float*)below, c->g);

@@ -57,11 +57,20 @@ __global__ void pack_gauge_kernel(R* __restrict__ native, const R* __restrict__ 
 // 8-real storage (fields.cuh): r = (Re a1, Im a1, Re a2, Im a2, Re b0, Im b0, arg(a0) / pi, arg(c0) / pi), the two
 // phases evaluated in double and rounded once.  Same grid as pack_gauge_kernel.
 template <typename R>
-__global__ void pack_gauge8_kernel(R* __restrict__ native, const R* __restrict__ canon, const R* __restrict__ below, Geom g) {
+__global__ void pack_gauge8_kernel(R* __restrict__ native, const R* __restrict__ canon, const R* __restrict__ below, Geom g,
+                                   double min_margin2, unsigned* __restrict__ bad) {
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
     if (cb >= g.Vh) return;
     const int k = blockIdx.y, p = blockIdx.z;
     const R* src = link_source<R>(canon, below, g, cb, p, k);
+    // the three squared moduli the decoder (recon8, fields.cuh) takes roots of and divides by: |U00|^2, N2 = |U01|^2 + |U02|^2,
+    // |U20|^2.  A link with one of them below min_margin2 cannot be decoded (unit links: N2 = 0 -> NaN): report it.
+    {
+        const double a0 = (double)src[0] * src[0] + (double)src[1] * src[1];
+        const double n2 = (double)src[2] * src[2] + (double)src[3] * src[3] + (double)src[4] * src[4] + (double)src[5] * src[5];
+        const double c0 = (double)src[12] * src[12] + (double)src[13] * src[13];
+        if (!(a0 >= min_margin2 && n2 >= min_margin2 && c0 >= min_margin2)) atomicOr(bad, 1u);   // a NaN fails every comparison
+    }
     constexpr double inv_pi = 0.31830988618379067154;
     R r[8] = {src[2], src[3], src[4], src[5], src[6], src[7],
               (R)(atan2((double)src[1], (double)src[0]) * inv_pi), (R)(atan2((double)src[13], (double)src[12]) * inv_pi)};

@@ -419,6 +419,25 @@ def test_recon8_links(H, precision):
     c = H.Gpu(dims, precision, 8, (1, 1, 1, -1), li.random_su3_links(dims, seed=3).astype(cd)).ctx
     assert c.gauge_recon8_margin(torch.from_numpy(li.unit_links(dims).astype(cd)).to("cuda:0"), scratch) == 0.0
     import paper_1112_5280_b200 as L
+    # ... and lqcd_pack_gauge refuses them instead of packing something the dslash turns into NaN: the whole unit field,
+    # a single unit link in an otherwise random field, one link with U00 = 0 (a cyclic permutation matrix), one NaN
+    good = li.random_su3_links(dims, seed=3).astype(cd)
+    one_unit, one_perm, one_nan = good.copy(), good.copy(), good.copy()
+    one_unit[2, 1, 3, 0, 2] = np.eye(3)
+    one_perm[1, 3, 2, 1, 0] = np.roll(np.eye(3), 1, axis=1)
+    one_nan[0, 0, 0, 0, 0, 0, 1] = np.nan
+    native = torch.empty(c.gauge_bytes(), dtype=torch.uint8, device="cuda:0")
+    for what, bad in (("unit field", li.unit_links(dims).astype(cd)), ("one unit link", one_unit),
+                      ("one permutation link", one_perm), ("one NaN", one_nan)):
+        with pytest.raises(L.LqcdError) as e:
+            c.pack_gauge(native, torch.from_numpy(np.ascontiguousarray(bad)).to("cuda:0"))
+            pytest.fail(f"recon 8: {what} was packed without complaint")
+        assert e.value.status == L.LQCD_EUNSUPPORTED, what
+    c.pack_gauge(native, torch.from_numpy(np.ascontiguousarray(good)).to("cuda:0"))   # the flag does not stick
+    # a cold start therefore goes through 12-real links and gives finite numbers (H psi = 8 psi for constant psi)
+    g12 = H.Gpu(dims, precision, 12, (1, 1, 1, 1), li.unit_links(dims).astype(cd))
+    const = np.ones(dims[::-1] + (4, 3), dtype=cd)
+    assert np.allclose(g12.dslash_full(const), 8 * const)
     with pytest.raises(L.LqcdError) as e:
         L.Context(dims, 16, 8)
     assert e.value.status == L.LQCD_EUNSUPPORTED
