@@ -216,8 +216,8 @@ class PeerMemoryTransport:
         assert self.ptrs[slab.rank] == self.buf.data_ptr()
         self.side = torch.cuda.Stream(self.device)
         self.epoch = 0
-        torch.cuda.synchronize(self.device)
-        dist.barrier()                          # every rank's flags are zero before anyone pushes
+        torch.cuda.synchronize(self.device)     # this rank's flags are zero; make_transport's agreement (a collective
+                                                # every rank passes) is what keeps anyone from pushing before that holds everywhere
 
     def _halo(self, rank, gen, which):          # which: 0 = from_up, 1 = from_down
         return self.ptrs[rank] + (2 * gen + which) * self.hb
@@ -246,15 +246,43 @@ def _p2p_name(dist):
     return "ncclSend/ncclRecv" if dist.get_backend() == "nccl" else f"{dist.get_backend()} send/recv through pinned host copies (functional test path)"
 
 
-def make_transport(slab, dist, device, kind="auto"):
-    """kind: "peer" (symmetric memory, fails loudly if unavailable), "sendrecv", or "auto" (peer memory if the process
-    group and the devices support it, else send/recv).  Returns (transport, name)."""
-    if kind in ("auto", "peer"):
-        try:
-            return PeerMemoryTransport(slab, dist, device), "peer-memory stores + device-side epoch flags (symmetric memory)"
-        except Exception as e:  # noqa: BLE001 -- any failure of the rendezvous means: no peer mapping on this box
-            if kind == "peer":
-                raise
-            why = f"{type(e).__name__}: {e}"
-            return SendRecvTransport(slab, dist, device), f"{_p2p_name(dist)} (peer memory unavailable: {why[:120]})"
-    return SendRecvTransport(slab, dist, device), _p2p_name(dist)
+def _all_ranks_ok(dist, ok, device):
+    """Collective: True on every rank iff `ok` is true on every rank (MIN over the group).  The tensor lives where the
+    backend can reduce it: on the GPU for NCCL, on the host otherwise."""
+    import torch
+    t = torch.tensor([1 if ok else 0], dtype=torch.int32, device=device if dist.get_backend() == "nccl" else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MIN)
+    return bool(int(t.item()))
+
+
+def make_transport(slab, dist, device, kind="auto", peer_factory=None):
+    """Returns (transport, name).  Collective: every rank of the group must call it with the same `kind`.
+
+    kind = "sendrecv"  ncclSend / ncclRecv between ring neighbours (gloo through pinned host copies in the CPU tests).
+    kind = "auto"      the same.  The peer-memory path has never run on two physical GPUs (every measurement of this
+                       repository is single-GPU), and its boundary kernels spin on flags another GPU
+                       writes, so it is not something to pick silently.
+    kind = "peer"      symmetric memory + device-side epoch flags (PeerMemoryTransport), or an exception ON EVERY RANK.
+    kind = "peer_or_sendrecv"  peer memory if it came up on every rank, send/recv on every rank otherwise.
+
+    The choice is agreed on by the whole group: each rank tries to set the peer path up, then a MIN all-reduce of the
+    outcome decides for all.  Without that, a rank whose rendezvous failed would post ncclSend / ncclRecv while its
+    neighbours store into peer memory and spin on flags that are never written -- a hang on one side, a trap on the
+    other.  (A rank that dies inside the rendezvous itself still stalls the others until the process group's timeout:
+    nothing after the fact can repair that.)  peer_factory: the constructor to try, for tests."""
+    if kind not in ("auto", "sendrecv", "peer", "peer_or_sendrecv"):
+        raise ValueError(f"unknown transport kind {kind!r}")
+    if kind in ("auto", "sendrecv"):
+        return SendRecvTransport(slab, dist, device), _p2p_name(dist)
+    transport, why = None, ""
+    try:
+        transport = (peer_factory or PeerMemoryTransport)(slab, dist, device)
+    except Exception as e:  # noqa: BLE001 -- any failure of the set-up means: no peer mapping for this rank
+        why = f"{type(e).__name__}: {e}"[:160]
+    if _all_ranks_ok(dist, transport is not None, device):
+        return transport, "peer-memory stores + device-side epoch flags (symmetric memory)"
+    transport = None    # drop a mapping that came up here but not everywhere
+    why = why or "set-up failed on another rank"
+    if kind == "peer":
+        raise RuntimeError(f"peer-memory transport unavailable on at least one rank (rank {slab.rank}: {why})")
+    return SendRecvTransport(slab, dist, device), f"{_p2p_name(dist)} (peer memory unavailable: {why})"

@@ -100,6 +100,60 @@ def test_time_slab_face_exchange_world4():
     _check_ring(4)
 
 
+def _transport_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    from paper_1112_5280_b200.slab import TimeSlab, SendRecvTransport, make_transport
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        s = TimeSlab((8, 8, 8, 16), 32, 12, (1, 1, 1, -1), rank, world)
+
+        class FakePeer:                       # stands in for PeerMemoryTransport: comes up on rank 0 only / everywhere
+            def __init__(self, slab, dist_, device, fail_on=()):
+                if slab.rank in fail_on:
+                    raise RuntimeError("no peer mapping on this rank")
+
+        res = {}
+        t, name = make_transport(s, dist, "cpu", "auto")
+        res["auto"] = type(t).__name__
+        t, name = make_transport(s, dist, "cpu", "peer_or_sendrecv", peer_factory=lambda *a: FakePeer(*a, fail_on=(1,)))
+        res["fallback"] = (type(t).__name__, "unavailable" in name)
+        t, name = make_transport(s, dist, "cpu", "peer_or_sendrecv", peer_factory=lambda *a: FakePeer(*a))
+        res["all_ok"] = type(t).__name__
+        try:
+            make_transport(s, dist, "cpu", "peer", peer_factory=lambda *a: FakePeer(*a, fail_on=(1,)))
+            res["peer"] = "returned"
+        except RuntimeError as e:
+            res["peer"] = "raised: " + str(e)
+        # the transport agreed on works: one ring exchange after the fallback
+        tr = make_transport(s, dist, "cpu", "peer_or_sendrecv", peer_factory=lambda *a: FakePeer(*a, fail_on=(0,)))[0]
+        tr.send_up.fill_(10 * rank + 1)
+        tr.send_down.fill_(10 * rank + 2)
+        tr.exchange(s)
+        res["exchange"] = (int(tr.from_up[0]), int(tr.from_down[0]))
+        out[rank] = res
+    finally:
+        dist.destroy_process_group()
+
+
+def test_transport_choice_is_agreed_on_by_every_rank_world2():
+    """make_transport: if the peer-memory set-up fails on ONE rank, both ranks use send/recv ("peer_or_sendrecv") or both
+    raise ("peer") -- never one rank spinning on peer flags while the other posts ncclSend.  "auto" is send/recv."""
+    world, port = 2, _free_port()
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_transport_worker, args=(world, port, out), nprocs=world, join=True)
+        res = dict(out)
+    for r in range(world):
+        assert res[r]["auto"] == "SendRecvTransport"
+        assert res[r]["fallback"] == ("SendRecvTransport", True), res[r]
+        assert res[r]["all_ok"] == "FakePeer"
+        assert res[r]["peer"].startswith("raised: peer-memory transport unavailable"), res[r]
+        other = 1 - r
+        assert res[r]["exchange"] == (10 * other + 2, 10 * other + 1)
+    assert "no peer mapping" in res[1]["peer"] and "another rank" in res[0]["peer"]
+
+
 def test_reference_arm_prints_the_contract_line():
     """bench.py --impl reference: one JSON line with the base contract's keys plus impl / cpu_baseline / e2e."""
     import json
