@@ -27,8 +27,29 @@ def sources():
     return units() + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [HEADER, os.path.abspath(__file__)]
 
 
+STAMP = LIB + ".flags"   # the flag string liblqcd.so was compiled with (git-ignored, travels with the library)
+
+
+def wanted_flags() -> str:
+    """What a build started now would pass to nvcc: the fixed flags plus $LQCD_NVCC_FLAGS (-D switches of a sweep)."""
+    return " ".join(NVCC_FLAGS + shlex.split(os.environ.get("LQCD_NVCC_FLAGS", "")))
+
+
+def built_flags():
+    """The flags of the library on disk, or None if it was built before the stamp existed / is missing."""
+    try:
+        with open(STAMP) as f:
+            return f.read().strip()
+    except OSError:
+        return None
+
+
 def stale() -> bool:
+    """Rebuild if the library is missing, older than a source, or was compiled with other flags than this process asks
+    for -- a library left behind by a tuning sweep (-DLQCD_...=...) must not be picked up by a default test or bench run."""
     if not os.path.exists(LIB):
+        return True
+    if built_flags() != wanted_flags():
         return True
     t = os.path.getmtime(LIB)
     return any(os.path.getmtime(s) > t for s in sources())
@@ -61,6 +82,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         tmp = LIB + f".tmp{tag}"
         subprocess.check_call([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *objs])
         os.replace(tmp, LIB)
+        with open(STAMP + f".tmp{tag}", "w") as f:
+            f.write(" ".join(NVCC_FLAGS + extra) + "\n")
+        os.replace(STAMP + f".tmp{tag}", STAMP)
     finally:
         for o in glob.glob(os.path.join(OBJ, f"*.{tag}.o")):
             os.remove(o)
