@@ -378,56 +378,6 @@ __device__ __forceinline__ void hop_step(typename Compute<S>::type acc[24],
     hop_rest<R, CBC, MU, FWD>(acc, h, scale, u, (crossmask >> K) & 1u, bc);
 }
 
-// Experiment (north_star (3) "warp shuffles where they pay"): the two x hops without a second
-// gather.  In the opposite-parity array the +-x neighbours of site cb are cb itself and cb + 1 (x odd) or cb - 1
-// (x even): every lane loads its "centre" spinor in[cb] once, projects it both ways (A = (1 - gamma_x) psi, what a
-// forward hop needs; B = (1 + gamma_x) psi, what a backward hop needs), keeps the one its own hop needs and hands the
-// other to the lane that needs it with 12 (fp32) / 24 (fp64) register shuffles.  A lane whose neighbour lives in
-// another warp tile gathers it from memory as before.  Off by default: measured slower.
-#ifndef LQCD_SHFL_X
-#define LQCD_SHFL_X 0
-#endif
-#ifndef LQCD_PREFETCH_TILE_LINKS
-#define LQCD_PREFETCH_TILE_LINKS 0
-#endif
-
-template <typename R>
-__device__ __forceinline__ R shfl_(R v, int src) { return __shfl_sync(0xffffffffu, v, src); }
-
-template <typename R, int RECON, bool CBC>
-__device__ __forceinline__ void hops_x_shuffled(R acc[24], const typename LinkStore<R, RECON>::word* __restrict__ site_links,
-                                                const R* __restrict__ in, int cb, int cb_end, int x_odd, const int nb[8],
-                                                unsigned crossmask, const BcPhases<R>& bc) {
-    R vc[24], A[12], B[12];
-    load_spinor<R>(in, cb, vc);
-    project<R, 0, +1>(vc, A);
-    project<R, 0, -1>(vc, B);
-    // the neighbour that is not the centre: forward (x odd) or backward (x even); its lane if it is in this warp's tile
-    const int other = x_odd ? nb[0] : nb[1];
-    const int src = other - (cb - (int)(threadIdx.x & 31u));   // lane l of the warp works on site (warp base + l)
-    const bool in_warp = src >= 0 && src < 32 && other < cb_end;  // ... if that site is inside this launch's range
-    R recv[12];
-#pragma unroll
-    for (int k = 0; k < 12; ++k) recv[k] = shfl_<R>(x_odd ? A[k] : B[k], in_warp ? src : 0);
-    // lanes handing to a lane of the other row kind would send the wrong projection: x_odd is constant along an x row
-    // and the neighbour is always in the same row, so sender and receiver agree.
-    if (!in_warp) {
-        R vo[24];
-        load_spinor<R>(in, other, vo);
-        if (x_odd) project<R, 0, +1>(vo, recv); else project<R, 0, -1>(vo, recv);
-    }
-    R hf[12], hb[12], u[18];
-#pragma unroll
-    for (int k = 0; k < 12; ++k) {
-        hf[k] = x_odd ? recv[k] : A[k];
-        hb[k] = x_odd ? B[k] : recv[k];
-    }
-    load_link<R, RECON>(site_links, 0, u);
-    hop_rest<R, CBC, 0, true>(acc, hf, (R)1, u, (crossmask >> 0) & 1u, bc);
-    load_link<R, RECON>(site_links, 1, u);
-    hop_rest<R, CBC, 0, false>(acc, hb, (R)1, u, (crossmask >> 1) & 1u, bc);
-}
-
 // Resident 64-thread blocks per SM promised to ptxas (__launch_bounds__ min blocks).  The hint sets the
 // register budget (65536 / (64 value)), and ptxas spends whatever budget it is given on hoisting the
 // gathers ahead of their use, so it fixes the balance between loads in flight per thread and threads
@@ -549,13 +499,7 @@ dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restr
         if (ty >= map.ny || tz >= g.Z || tt >= g.T) return;   // boxes that stick out of the lattice (warp-uniform)
         cb = (ty + map.ny * (tz + g.Z * tt)) * TILE + (int)(threadIdx.x & 31u);
     }
-    constexpr bool SHFLX = LQCD_SHFL_X && sizeof(S) != 2 && !half_links<S, RECON>;
-    bool live = true;
-    if (cb >= cb_end) {
-        if constexpr (!SHFLX) return;
-        live = false;     // with shuffles every lane of the warp stays: a dead lane works on the last site and stores nothing
-        cb = cb_end - 1;
-    }
+    if (cb >= cb_end) return;
     const Site s = decode_site(g, cb, p);
 
     // K1: all eight neighbours and boundary-crossing flags
@@ -565,22 +509,12 @@ dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restr
     const auto* site_links = reinterpret_cast<const typename LinkStore<S, RECON>::word*>(gauge) +
                              LinkStore<S, RECON>::word0(g.ntiles, p, cb, 0);
 
-#if LQCD_PREFETCH_TILE_LINKS   // experiment: one bulk L2 prefetch of the warp tile's whole link block (8 hops, contiguous) up front
-    if ((threadIdx.x & 31u) == 0) {
-        constexpr unsigned bytes = 8u * (RECON == RECON_12H ? 12 : RECON) / LinkStore<S, RECON>::R_PER_WORD * TILE * sizeof(typename LinkStore<S, RECON>::word);
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(site_links), "r"(bytes) : "memory");
-    }
-#endif
     R acc[24];
 #pragma unroll
     for (int k = 0; k < 24; ++k) acc[k] = 0;
 
-    if constexpr (SHFLX) {
-        hops_x_shuffled<R, RECON, CBC>(acc, site_links, in, cb, cb_end, s.x_odd, nb, crossmask, bc);
-    } else {
-        hop_step<S, RECON, CBC, 0>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
-        hop_step<S, RECON, CBC, 1>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
-    }
+    hop_step<S, RECON, CBC, 0>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
+    hop_step<S, RECON, CBC, 1>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
     hop_step<S, RECON, CBC, 2>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
     hop_step<S, RECON, CBC, 3>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
     hop_step<S, RECON, CBC, 4>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
@@ -588,7 +522,7 @@ dslash_kernel(S* __restrict__ out, const S* __restrict__ gauge, const S* __restr
     hop_step<S, RECON, CBC, 6>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
     hop_step<S, RECON, CBC, 7>(acc, site_links, in, g.ntiles, nb, crossmask, bc);
 
-    finish_site<S, EPI>(acc, out, xin, epi, g.ntiles, cb, live);
+    finish_site<S, EPI>(acc, out, xin, epi, g.ntiles, cb, true);
 }
 
 }  // namespace lqcd

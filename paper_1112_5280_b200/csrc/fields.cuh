@@ -55,27 +55,11 @@ __device__ __forceinline__ void unpack(const double4_& w, double* v) {
     for (int i = 0; i < 4; ++i) v[i] = w.v[i];
 }
 
-// cache-policy experiments: spinor gathers 0 = default, 1 = L2::evict_last; 256-bit link words 0 =
-// default read-only path, 1 = .cs (evict-first), 2 = nc.L1::no_allocate.L2::evict_first; stores 0 = default, 1 = .cs
-#ifndef LQCD_SPINOR_POLICY
-#define LQCD_SPINOR_POLICY 0
-#endif
-#ifndef LQCD_LINK256_POLICY
-#define LQCD_LINK256_POLICY 0
-#endif
-#ifndef LQCD_STORE_POLICY
-#define LQCD_STORE_POLICY 0
-#endif
-#if LQCD_SPINOR_POLICY == 1
-#define LQCD_LD_SPINOR "ld.global.nc.L2::evict_last"
-#else
+// Cache policy of the field accesses: plain read-only (.nc) gathers and default stores.  L2::evict_last on the spinor
+// gathers, .cs / L1::no_allocate.L2::evict_first on the 256-bit link words and .cs stores were each measured within
+// +-0.5 % of this and are not kept as switches.
 #define LQCD_LD_SPINOR "ld.global.nc"
-#endif
-#if LQCD_STORE_POLICY == 1
-#define LQCD_ST_SPINOR "st.global.cs"
-#else
 #define LQCD_ST_SPINOR "st.global"
-#endif
 __device__ __forceinline__ float8_ ldg256(const float8_* p) {
     float8_ w;
     asm(LQCD_LD_SPINOR ".v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
@@ -90,13 +74,7 @@ __device__ __forceinline__ double4_ ldg256(const double4_* p) {
 // 256-bit link words (fp64 12-real / 8-real storage): read exactly once per application
 __device__ __forceinline__ double4_ ldg256_stream(const double4_* p) {
     double4_ w;
-#if LQCD_LINK256_POLICY == 1
-    asm("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(w.v[0]), "=d"(w.v[1]), "=d"(w.v[2]), "=d"(w.v[3]) : "l"(p));
-#elif LQCD_LINK256_POLICY == 2
-    asm("ld.global.nc.L1::no_allocate.L2::evict_first.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(w.v[0]), "=d"(w.v[1]), "=d"(w.v[2]), "=d"(w.v[3]) : "l"(p));
-#else
     asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(w.v[0]), "=d"(w.v[1]), "=d"(w.v[2]), "=d"(w.v[3]) : "l"(p));
-#endif
     return w;
 }
 // Plain (coherent) 256-bit loads for operands the same kernel overwrites (the in-place BLAS-1 updates): .nc is only

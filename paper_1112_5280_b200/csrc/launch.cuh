@@ -2,8 +2,7 @@
 // instantiation units inst_*.cu (one per storage type x link format, so that the library builds in parallel:
 // each unit instantiates dslash_kernel for its 4 epilogues x 2 boundary-phase kinds).
 #pragma once
-#include <cstdio>
-#include <cstdlib>
+#include <atomic>
 #include <mutex>
 
 #include "../../include/lqcd.h"
@@ -26,7 +25,7 @@ struct lqcd_ctx {
     lqcd_params p;
     lqcd::Geom g;
     bool complex_bc;
-    int kernel;   // LQCD_KERNEL_GATHER, _PIPE or _BLOCKED (lqcd_set_kernel)
+    int kernel;   // LQCD_KERNEL_GATHER, _PIPE, _BLOCKED or _LSTAGE (lqcd_set_kernel)
     mutable lqcd_host_pipe host;
 };
 
@@ -60,14 +59,24 @@ BcPhases<R> make_bc(const lqcd_ctx* c) {
 // the pipelined kernel exists for fp32 / fp64 fields with links stored in the same precision
 template <typename S, int RECON> constexpr bool pipe_capable = (sizeof(S) == 4 || sizeof(S) == 8) && (RECON == 8 || RECON == 12 || RECON == 18);
 
+// Per-device launch state.  One process may drive several GPUs through the C ABI, so anything cached about "the device"
+// is indexed by the current device's ordinal; entries are atomics because two host threads may launch at once (both then
+// write the same value, which is harmless).
+constexpr int MAX_DEVICES = 64;
+
+inline int current_device() {
+    int dev = -1;
+    return cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < MAX_DEVICES ? dev : -1;
+}
+
 // SMs of the current device (persistent grid of the pipelined kernel); 0 on error
 inline int sm_count() {
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0, v = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess) n = v;
-    }
-    return n;
+    static std::atomic<int> n[MAX_DEVICES];
+    const int dev = current_device();
+    if (dev < 0) return 0;
+    int v = n[dev].load(std::memory_order_relaxed);
+    if (v == 0 && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess) n[dev].store(v, std::memory_order_relaxed);
+    return v;
 }
 
 template <typename R, int RECON, int EPI, bool CBC>
@@ -75,10 +84,13 @@ lqcd_status launch_pipe(const lqcd_ctx* c, void* out, const void* gauge, const v
                         const EpiArgs& e, int parity, cudaStream_t st, CbRange rg) {
     using P = Pipe<R, RECON>;
     auto kernel = dslash_pipe_kernel<R, RECON, EPI, CBC>;
-    static bool configured = false;
-    if (!configured) {
+    // the opt-in to more than 48 KB of dynamic shared memory is a property of the kernel ON ONE DEVICE: once per device
+    static std::atomic<bool> configured[MAX_DEVICES];
+    const int dev = current_device();
+    if (dev < 0) return LQCD_ECUDA;
+    if (!configured[dev].load(std::memory_order_acquire)) {
         if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, P::SMEM_BYTES) != cudaSuccess) return after_launch();
-        configured = true;
+        configured[dev].store(true, std::memory_order_release);
     }
     const int nt = ((rg.end + TILE - 1) >> 5) - (rg.begin >> 5), nwork = parity < 0 ? 2 * nt : nt;
     const int nsm = sm_count();
@@ -90,17 +102,13 @@ lqcd_status launch_pipe(const lqcd_ctx* c, void* out, const void* gauge, const v
 }
 
 // Box of nwarps warp tiles for the blocked map: 2 tiles along y and 2 along t where the block has the warps for it, the
-// rest along z ($LQCD_BOX = "by,bz,bt" overrides, for sweeps).
+// rest along z (by * bz * bt = nwarps for the warp counts in use: 16, 12, 8; other shapes were swept in round 2).
 inline BlockMap box_shape(int nwarps, const Geom& g) {
     BlockMap m;
     m.ny = g.sz / TILE;
     m.by = nwarps >= 4 && m.ny >= 2 ? 2 : 1;
     m.bt = nwarps >= 8 ? 2 : 1;
     m.bz = nwarps / (m.by * m.bt);
-    if (const char* e = std::getenv("LQCD_BOX")) {
-        int a, b, c2;
-        if (std::sscanf(e, "%d,%d,%d", &a, &b, &c2) == 3 && a > 0 && b > 0 && c2 > 0 && a * b * c2 <= nwarps) { m.by = a; m.bz = b; m.bt = c2; }
-    }
     m.gy = (m.ny + m.by - 1) / m.by;
     m.gz = (g.Z + m.bz - 1) / m.bz;
     return m;
@@ -140,16 +148,6 @@ lqcd_status launch_one(const lqcd_ctx* c, void* out, const void* gauge, const vo
     }
     constexpr int BLOCK = DSLASH_BLOCK;
     const dim3 grid((rg.end - rg.begin + BLOCK - 1) / BLOCK, parity < 0 ? 2 : 1);
-#ifdef LQCD_CARVEOUT_EXPERIMENT   // how much L1 the gather kernel needs: $LQCD_CARVEOUT = per cent of the 228 KB given to shared memory
-    {
-        static int done = 0;
-        if (!done) {
-            if (const char* e = std::getenv("LQCD_CARVEOUT"))
-                cudaFuncSetAttribute(dslash_kernel<S, RECON, EPI, CBC, BLOCK>, cudaFuncAttributePreferredSharedMemoryCarveout, std::atoi(e));
-            done = 1;
-        }
-    }
-#endif
     dslash_kernel<S, RECON, EPI, CBC, BLOCK><<<grid, BLOCK, 0, st>>>(
         (S*)out, (const S*)gauge, (const S*)in, (const S*)xin, epi, c->g, parity < 0 ? 0 : parity, make_bc<A>(c), rg.begin, rg.end, BlockMap{0, 0, 0, 0, 0, 0});
     return after_launch();

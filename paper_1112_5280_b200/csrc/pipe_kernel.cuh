@@ -107,11 +107,6 @@ __device__ __forceinline__ unsigned long long policy_evict_first() {
     return p;
 }
 
-// experiments only (results are wrong): 1 = no arithmetic, 2 = no copies
-#ifndef LQCD_PIPE_DEBUG
-#define LQCD_PIPE_DEBUG 0
-#endif
-
 // ---- sizes ------------------------------------------------------------------------------------------------------------
 // consumer warps per CTA (plus 4 producer warps).  fp32: 4 + 12 warps of 128 registers; fp64: 4 + 8 warps of 168.
 #ifndef LQCD_PIPE_CONSUMERS_F32
@@ -303,10 +298,6 @@ __device__ __forceinline__ void consume_tile(R acc[24], char* smem, unsigned bar
         lds_link<R, RECON>(slot, 1, lane, rb);
         __syncwarp();                             // every lane's shared-memory reads of the chunk are in registers
         if (lane == 0) asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(released), "r"(use + 1u) : "memory");
-#if LQCD_PIPE_DEBUG == 1   // staging only: keep the loads alive, skip the arithmetic (bandwidth of the data path alone)
-#pragma unroll
-        for (int k = 0; k < 12; ++k) acc[k] += hf[k] + hb[k] + rf[k % RECON] + rb[k % RECON];
-#else
         R u[18], chi[12];
         const unsigned cross = crossmask >> (2 * mu);
         decode_link<R, RECON>(rf, u);
@@ -317,7 +308,6 @@ __device__ __forceinline__ void consume_tile(R acc[24], char* smem, unsigned bar
         f = boundary_phase<R, CBC>(hb, (R)1, (cross >> 1) & 1u, br, -bi);
         su3_multiply<R, false>(hb, u, chi);
         reconstruct_accumulate_mu<R, -1>(mu, acc, chi, f);
-#endif
     }
 }
 
@@ -356,15 +346,6 @@ __device__ __forceinline__ void produce_direction(char* smem, unsigned bars, uns
         }
         const unsigned dst = ring + slot * (unsigned)P::chunk_bytes(MU), tiles = dst + 2 * P::LINK_BYTES;
         const unsigned full = bars + 8 * (MU * P::DEPTH + slot), released = rels + 4 * (MU * P::DEPTH + slot);
-#if LQCD_PIPE_DEBUG == 2   // no copies: the consumers run on whatever shared memory holds (their speed alone)
-        if (elect_one()) {
-            await_released(released, use);
-            mbar_arrive(full);
-        }
-        __syncwarp();
-        if (++slot == P::DEPTH) { slot = 0; ++use; }
-        continue;
-#endif
         if (elect_one()) {
             await_released(released, use);        // the slot's previous chunk has been consumed
             mbar_arrive_expect_tx(full, 2 * P::LINK_BYTES + ((t0 >= 0) + (t1 >= 0) + (t2 >= 0)) * P::TILE_BYTES);
