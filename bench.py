@@ -589,7 +589,9 @@ def heatbath_leg(torch, dev, cfg_id=4, beta=6.0, ntries=4, sweeps=3):
     ws = torch.empty(ctx.plaquette_workspace_bytes(), dtype=torch.uint8, device=dev)
     p0 = ctx.plaquette(U, ws)
     n = ctx.heatbath_uniforms(ntries)
-    u = [1.0 - torch.rand(n, dtype=torch.float64, device=dev) for _ in range(2)]
+    # one independent array of uniforms per sublattice launch of a sweep (8 x 453 MB at 32^3 x 64, ntries 4), redrawn
+    # between sweeps outside the timed region: no number is used twice, so plaquette_after is a heatbath's, not an artefact
+    u = [1.0 - torch.rand(n, dtype=torch.float64, device=dev) for _ in range(8)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     times = []
     for s in range(sweeps + 1):
@@ -597,7 +599,7 @@ def heatbath_leg(torch, dev, cfg_id=4, beta=6.0, ntries=4, sweeps=3):
         e0.record()
         for mu in range(4):
             for parity in (0, 1):
-                ctx.heatbath_sublattice(U, beta, mu, parity, u[(mu + parity) & 1], ntries)
+                ctx.heatbath_sublattice(U, beta, mu, parity, u[2 * mu + parity], ntries)
         e1.record()
         torch.cuda.synchronize()
         times.append(e0.elapsed_time(e1))

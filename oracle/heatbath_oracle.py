@@ -27,6 +27,12 @@ Random numbers are INPUTS (the method's uniforms are passed in by the caller, th
 CUDA path): uniforms[site cb of the sublattice][subgroup 3][4 ntries + 2], the 4 numbers of attempt t at [4 t, 4 t + 4),
 the two direction numbers last.  Links are periodic and carry no boundary phase (reading A6).
 Arrays: links [4][T][Z][Y][X][3][3] complex128 (canonical layout).  Imports nothing from paper_1112_5280_b200.
+
+  reunitarise  every update multiplies a link by a rounded SU(2) element, so over many sweeps the links drift off the
+             group by accumulated rounding.  The standard cure (reading F8; it is the "Gram-Schmidt
+             reunitarised" construction BASELINE.json's configs name for the random links) projects a link back:
+                 row0 <- row0 / |row0|;  row1 <- row1 - <row0, row1> row0, then / |row1|;  row2 <- conj(row0 x row1)
+             which is unitary with det = +1 by construction and leaves an exact SU(3) matrix unchanged.
 """
 from __future__ import annotations
 
@@ -150,3 +156,17 @@ def sweep(U: np.ndarray, beta: float, rng: np.random.Generator, ntries: int = 8)
             u = 1.0 - rng.random((Vh, 3, 4 * ntries + 2))
             U = heatbath_sublattice(U, beta, mu, parity, u)
     return U
+
+
+def reunitarise(U: np.ndarray) -> np.ndarray:
+    """Project every 3x3 matrix of U[..., 3, 3] back to SU(3): Gram-Schmidt on rows 0 and 1 in this order, with
+    <a, b> = sum_k conj(a_k) b_k, then row 2 = conj(row 0 x row 1).  Returns a new array."""
+    U = np.asarray(U, dtype=np.complex128)
+    r0 = U[..., 0, :]
+    r0 = r0 / np.sqrt(np.sum(np.abs(r0) ** 2, axis=-1, keepdims=True))
+    r1 = U[..., 1, :]
+    r1 = r1 - np.sum(np.conj(r0) * r1, axis=-1, keepdims=True) * r0
+    r1 = r1 / np.sqrt(np.sum(np.abs(r1) ** 2, axis=-1, keepdims=True))
+    r2 = np.conj(np.cross(r0, r1))
+    return np.stack([r0, r1, r2], axis=-2)
+

@@ -11,6 +11,9 @@ the definitions and the mathematics fix, none of it computed by the oracle's own
       Re tr of the block of G W equals 2 k a0
   H5  physics at both ends of the coupling: strong coupling <P> = beta/18 + O(beta^2), weak coupling (equipartition of the
       24 non-gauge degrees of freedom per site over 6 plaquettes) <1 - P> = 2/beta + O(1/beta^2)
+  H6  reunitarise: the result is in SU(3) for arbitrary input; an SU(3) matrix is a fixed point; a perturbed one moves by
+      no more than the perturbation's order; rows 0 and 1 are what a library QR of U^+ gives (Gram-Schmidt on the rows
+      of U is the QR factorisation of U^+ with a positive real diagonal of R); one hand-worked matrix
 """
 import numpy as np
 import pytest
@@ -171,3 +174,34 @@ def test_H5_strong_and_weak_coupling_plaquette():
         if s >= 20:
             P.append(hb.plaquette(U))
     assert abs((1 - np.mean(P)) * beta / 2 - 1.0) <= 0.08, (1 - np.mean(P)) * beta / 2
+
+
+def test_H6_reunitarise_projects_to_su3():
+    rng = np.random.default_rng(66)
+    # (i) arbitrary complex matrices end up unitary with det = +1
+    A = rng.standard_normal((500, 3, 3)) + 1j * rng.standard_normal((500, 3, 3))
+    P = hb.reunitarise(A)
+    assert np.abs(P @ np.conj(np.swapaxes(P, -1, -2)) - np.eye(3)).max() < 5e-15
+    assert np.abs(np.linalg.det(P) - 1.0).max() < 5e-15
+    # (ii) rows 0 and 1 against the library QR of A^+ : A^+ = Q R  =>  rows of A = R^+ Q^+, so with the phases of diag(R)
+    # removed the rows of Q^+ are the Gram-Schmidt rows.  (Row 2 is fixed by det = +1, checked in (i).)
+    for a, p in zip(A[:50], P[:50]):
+        Q, R = np.linalg.qr(np.conj(a.T))
+        ph = np.diag(R) / np.abs(np.diag(R))
+        rows = np.conj((Q * ph).T)
+        assert np.abs(rows[:2] - p[:2]).max() < 1e-13
+    # (iii) SU(3) matrices are fixed points; a perturbation of size d moves the projection by O(d) and not more
+    U = li.random_su3_links((4, 4, 4, 4), seed=9)
+    assert np.abs(hb.reunitarise(U) - U).max() < 1e-15
+    d = 1e-9
+    noisy = U + d * (rng.standard_normal(U.shape) + 1j * rng.standard_normal(U.shape))
+    back = hb.reunitarise(noisy)
+    assert 0 < np.abs(back - U).max() < 20 * d
+    assert np.abs(back @ np.conj(np.swapaxes(back, -1, -2)) - np.eye(3)).max() < 5e-15
+    # (iv) by hand: rows (2, 0, 0), (1, 1, 0), anything -> e0, e1, and e0 x e1 = e2 (real, so conj changes nothing);
+    # with a phase on row 0: row0 = i e0, row1 = e1  =>  row2 = conj(i e0 x e1) = conj(i e2) = -i e2, det = i * 1 * (-i) = 1
+    M = np.array([[2, 0, 0], [1, 1, 0], [7, 7, 7]], dtype=complex)
+    assert np.allclose(hb.reunitarise(M), np.eye(3), atol=1e-15)
+    M = np.array([[3j, 0, 0], [5, 2, 0], [0, 0, 0]], dtype=complex)
+    assert np.allclose(hb.reunitarise(M), np.diag([1j, 1, -1j]), atol=1e-15)
+
