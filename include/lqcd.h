@@ -298,6 +298,12 @@ lqcd_status lqcd_unpack_update_links(const lqcd_ctx* ctx, void* canonical_dev, c
 size_t lqcd_heatbath_uniforms(const lqcd_ctx* ctx, int ntries);
 lqcd_status lqcd_heatbath_sublattice(const lqcd_ctx* ctx, void* links_update_dev, double beta, int mu, int parity,
                                      const void* uniforms_dev, int ntries, void* stream);
+/* Projects every link of a field in the update layout back to SU(3), in place (reading F8): row 0 normalised,
+ * row 1 orthogonalised against it and normalised, row 2 = conj(row 0 x row 1).  Every sublattice update multiplies a
+ * link by a rounded SU(2) element, so over many sweeps the links drift off the group, and 12- / 8-real storage assumes
+ * det = 1 and unitarity exactly: call this every few sweeps and before lqcd_unpack_update_links + lqcd_pack_gauge.
+ * A link that already is in SU(3) changes by rounding only.  One launch, asynchronous on `stream`; precision 64. */
+lqcd_status lqcd_reunitarise_links(const lqcd_ctx* ctx, void* links_update_dev, void* stream);
 size_t lqcd_plaquette_workspace_bytes(const lqcd_ctx* ctx);
 lqcd_status lqcd_plaquette(const lqcd_ctx* ctx, const void* links_update_dev, void* workspace_dev, double* plaq_host,
                            void* stream);

@@ -24,7 +24,7 @@ EXPORTS = [
     "lqcd_gauge_recon8_margin", "lqcd_set_kernel", "lqcd_selftest_fastdiv", "lqcd_update_links_bytes", "lqcd_pack_update_links", "lqcd_unpack_update_links",
     "lqcd_heatbath_uniforms", "lqcd_heatbath_sublattice",
     "lqcd_plaquette_workspace_bytes", "lqcd_plaquette", "lqcd_status_string", "lqcd_last_cuda_error",
-    "lqcd_static_scratch_bytes", "lqcd_apply_M_eo_static",
+    "lqcd_static_scratch_bytes", "lqcd_apply_M_eo_static", "lqcd_reunitarise_links",
 ]
 
 
@@ -81,6 +81,7 @@ def _lib():
         lib.lqcd_heatbath_uniforms.argtypes = [vp, ci]
         lib.lqcd_heatbath_uniforms.restype = sz
         lib.lqcd_heatbath_sublattice.argtypes = [vp, vp, cd, ci, ci, vp, ci, vp]
+        lib.lqcd_reunitarise_links.argtypes = [vp, vp, vp]
         lib.lqcd_plaquette_workspace_bytes.argtypes = [vp]
         lib.lqcd_plaquette_workspace_bytes.restype = sz
         lib.lqcd_plaquette.argtypes = [vp, vp, vp, ctypes.POINTER(cd), vp]
@@ -200,6 +201,9 @@ class Context:
     def heatbath_sublattice(self, links, beta, mu, parity, uniforms, ntries, stream=None):
         _chk(_lib().lqcd_heatbath_sublattice(self._h, _ptr(links), float(beta), int(mu), int(parity), _ptr(uniforms),
                                              int(ntries), _stream(stream)), "lqcd_heatbath_sublattice")
+
+    def reunitarise_links(self, links, stream=None):
+        _chk(_lib().lqcd_reunitarise_links(self._h, _ptr(links), _stream(stream)), "lqcd_reunitarise_links")
 
     def plaquette_workspace_bytes(self): return _lib().lqcd_plaquette_workspace_bytes(self._h)
 

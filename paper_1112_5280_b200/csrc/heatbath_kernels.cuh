@@ -259,6 +259,46 @@ __global__ void __launch_bounds__(HB_BLOCK) plaquette_kernel(const double2* __re
     }
 }
 
+// Reunitarisation (reading F8), in place on the update layout; grid (ceil(Vh / block), 4 directions, 2 parities),
+// one link per thread:  row0 /= |row0|;  row1 -= <row0, row1> row0, /= |row1|;  row2 = conj(row0 x row1).
+__global__ void __launch_bounds__(HB_BLOCK) reunitarise_kernel(double2* links, Geom g) {
+    const int cb = blockIdx.x * HB_BLOCK + threadIdx.x;
+    if (cb >= g.Vh) return;
+    double2* w = links + update_word0(g.ntiles, blockIdx.y, blockIdx.z, cb);
+    const size_t Vp = (size_t)TILE * g.ntiles;
+    double2 a[3], b[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { a[k] = w[k * Vp]; b[k] = w[(3 + k) * Vp]; }
+    double n = 0.0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) n += a[k].x * a[k].x + a[k].y * a[k].y;
+    n = 1.0 / sqrt(n);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { a[k].x *= n; a[k].y *= n; }
+    double pr = 0.0, pi = 0.0;   // <row0, row1> = sum conj(a_k) b_k
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { pr += a[k].x * b[k].x + a[k].y * b[k].y; pi += a[k].x * b[k].y - a[k].y * b[k].x; }
+    n = 0.0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        b[k].x -= pr * a[k].x - pi * a[k].y;
+        b[k].y -= pr * a[k].y + pi * a[k].x;
+        n += b[k].x * b[k].x + b[k].y * b[k].y;
+    }
+    n = 1.0 / sqrt(n);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { b[k].x *= n; b[k].y *= n; }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const int i = (k + 1) % 3, j = (k + 2) % 3;   // (a x b)_k = a_i b_j - a_j b_i, then conjugated
+        const double cr = (a[i].x * b[j].x - a[i].y * b[j].y) - (a[j].x * b[i].x - a[j].y * b[i].y);
+        const double ci = (a[i].x * b[j].y + a[i].y * b[j].x) - (a[j].x * b[i].y + a[j].y * b[i].x);
+        w[k * Vp] = a[k];
+        w[(3 + k) * Vp] = b[k];
+        w[(6 + k) * Vp] = make_double2(cr, -ci);
+    }
+}
+
 // canonical [mu][V][3][3] complex128 <-> update layout; grid (ceil(Vh / block), 4 directions, 2 parities)
 template <bool UNPACK>
 __global__ void __launch_bounds__(HB_BLOCK) update_links_pack_kernel(double2* native, double2* canon, Geom g) {

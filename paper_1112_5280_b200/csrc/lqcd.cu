@@ -747,6 +747,14 @@ lqcd_status lqcd_unpack_update_links(const lqcd_ctx* c, void* canon, const void*
     return update_links_convert(c, const_cast<void*>(native), canon, stream, true);
 }
 
+lqcd_status lqcd_reunitarise_links(const lqcd_ctx* c, void* links, void* stream) {
+    if (!c || !links) return LQCD_EINVAL;
+    if (c->p.precision != 64) return LQCD_EUNSUPPORTED;
+    if (!aligned16(links)) return LQCD_EALIGN;
+    reunitarise_kernel<<<dim3((c->g.Vh + HB_BLOCK - 1) / HB_BLOCK, 4, 2), HB_BLOCK, 0, (cudaStream_t)stream>>>((double2*)links, c->g);
+    return after_launch();
+}
+
 size_t lqcd_heatbath_uniforms(const lqcd_ctx* c, int ntries) {
     return c && ntries > 0 ? (size_t)c->g.Vh * 3 * (4 * (size_t)ntries + 2) : 0;
 }

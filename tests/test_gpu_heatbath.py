@@ -108,3 +108,51 @@ def test_heatbath_error_codes():
         c32.heatbath_sublattice(Ud, 5.0, 0, 0, u, 2)
     assert e.value.status == L.LQCD_EUNSUPPORTED
     assert np.array_equal(links.get(), U)   # nothing was launched
+
+
+def _group_defect(U):
+    M = U.reshape(-1, 3, 3)
+    return max(np.abs(M @ np.conj(np.swapaxes(M, -1, -2)) - np.eye(3)).max(), np.abs(np.linalg.det(M) - 1.0).max())
+
+
+def test_reunitarise_links_matches_oracle_and_stops_the_drift():
+    """lqcd_reunitarise_links against oracle.reunitarise (reading F8, pin H6): on links pushed off the group by a 1e-6
+    perturbation (ragged lattice: the last tile is padded), and on the field 100 free-running GPU sweeps leave behind,
+    whose rounding drift the projection removes.  12-real storage of the projected field then reproduces its third row."""
+    dims = (6, 4, 6, 10)                     # V/2 = 720: not a multiple of the 32-site tile
+    L, ctx, U, dev = _setup(dims, 63)
+    rng = np.random.default_rng(11)
+    noisy = U + 1e-6 * (rng.standard_normal(U.shape) + 1j * rng.standard_normal(U.shape))
+    Ud = _Links(ctx, noisy, dev)
+    ctx.reunitarise_links(Ud.buf)
+    got, ref = Ud.get(), hb.reunitarise(noisy)
+    assert np.abs(got - ref).max() <= 1e-14
+    assert _group_defect(got) <= 1e-14 and _group_defect(noisy) > 1e-7
+    # a field in SU(3) is a fixed point up to rounding
+    Ud.put(U)
+    ctx.reunitarise_links(Ud.buf)
+    same = Ud.get()
+    assert np.abs(same - hb.reunitarise(U)).max() <= 1e-14
+    assert np.abs(same - U).max() <= 1e-13           # by as much as the generator's U is off the group, i.e. rounding
+
+    # 100 sweeps on 4^4 at beta = 6 without any projection, then one
+    dims, beta, ntries = (4, 4, 4, 4), 6.0, 4
+    L, ctx, U, dev = _setup(dims, 64)
+    Ud = _Links(ctx, U, dev)
+    n = ctx.heatbath_uniforms(ntries)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(1234)
+    for sweep in range(100):
+        for mu in range(4):
+            for parity in (0, 1):
+                u = 1.0 - torch.rand(n, dtype=torch.float64, device=dev, generator=gen)
+                ctx.heatbath_sublattice(Ud.buf, beta, mu, parity, u, ntries)
+    drifted = Ud.get()
+    d0 = _group_defect(drifted)
+    assert np.isfinite(drifted.view(np.float64)).all() and d0 < 1e-10       # 2400 rounded SU(2) multiplications per link
+    ctx.reunitarise_links(Ud.buf)
+    fixed = Ud.get()
+    assert _group_defect(fixed) <= 1e-14 and _group_defect(fixed) <= max(d0, 4e-15)
+    assert np.abs(fixed - hb.reunitarise(drifted)).max() <= 1e-14
+    assert np.abs(fixed - drifted).max() <= 4 * d0 + 1e-14                   # the projection moves a link by the drift, not more
+    assert np.abs(np.conj(np.cross(fixed[..., 0, :], fixed[..., 1, :])) - fixed[..., 2, :]).max() <= 5e-15   # what recon 12 rebuilds
